@@ -1,0 +1,351 @@
+/*
+ * sph_oracle.c -- TEST INFRASTRUCTURE, NOT THE PRODUCT.
+ *
+ * Plain, slow, single-threaded CPU restatement of the per-iteration hot path of the
+ * particle-decomposition SPH scheme of Unfer, Colle & Limido (arxiv 2310.03596,
+ * /root/reference/PAPER.md).  Every real quantity is fp64 (fp32 inputs are widened), except the
+ * bucket hash, whose operation sequence is pinned in fp32 (reading S2) so that the
+ * integer outputs have exactly one correct value.
+ *
+ * Only tests/, __graft_entry__.smoke() and bench.py's cpu_baseline / --impl reference legs may
+ * call this file.  It shares no code, header, table or constant with the CUDA path under
+ * paper_2310_03596_b200/csrc/ and includes nothing from include/.
+ *
+ * Build: gcc -O2 -ffp-contract=off -fno-fast-math -shared -fPIC (see oracle/build.py).
+ *
+ * Citations: "PAPER.md:N" = line N of /root/reference/PAPER.md; "S#"/"O#"/"I#" = the readings,
+ * oracle steps and invariants listed in DESIGN.md section 3 (taken from SURVEY.md section 8(c)).
+ *
+ * Pins (tests/test_oracle_pins.py, -m "not gpu"): brute-force O(N^2) neighbour / owner
+ * enumeration, kernel normalisation integral and dW/dr by finite differences, exact momentum
+ * conservation, zero rates for uniform translation, continuum limits of the gradient operators
+ * (sign and index conventions), Hooke / Jaumann textbook cases, expm() finite rotation,
+ * cell-table identities, sort vs numpy.lexsort, hash at bucket faces.  No function is unpinned.
+ */
+#include <math.h>
+#include <stdint.h>
+#include <stdlib.h>
+#include <string.h>
+
+#define ORC_GARBAGE 0xFFFFFFFFu /* S8: "some garbage collector hash" := 2^32-1 */
+
+/* ------------------------------------------------------------------------------------------
+ * O1  Bucket hash ("cubic buckets of size 2h ... Each particle is given a hash
+ * number corresponding to the bucket in which it is located"; PAPER.md:19 step a).
+ * Reading S1: linear index, x fastest.  Reading S2: the fp32 sequence sub, mul, floor, clamp.
+ * posm is [n][4] = x,y,z,m.
+ * ---------------------------------------------------------------------------------------- */
+void orc_hash(int64_t n, const float *posm, const float *origin, const int32_t *dims, float h,
+              uint32_t *hash)
+{
+    const float edge = 2.0f * h;    /* bucket edge 2h */
+    const float inv = 1.0f / edge;  /* rounded once, fp32 (S2)      */
+    for (int64_t i = 0; i < n; ++i) {
+        uint32_t c[3];
+        for (int a = 0; a < 3; ++a) {
+            float t = posm[4 * i + a] - origin[a];
+            float u = t * inv;
+            float f = floorf(u);
+            float top = (float)(dims[a] - 1);
+            if (f < 0.0f) f = 0.0f;      /* S3: out-of-grid particles are clamped */
+            if (f > top) f = top;
+            c[a] = (uint32_t)(int32_t)f;
+        }
+        hash[i] = c[0] + (uint32_t)dims[0] * (c[1] + (uint32_t)dims[1] * c[2]);
+    }
+}
+
+/* ------------------------------------------------------------------------------------------
+ * O2  Sort ("The particles are then sorted with respect to this hash number by
+ * the radix sort algorithm").  Reading S5: the key is (hash, particle id), ids are 0..n-1.
+ * The oracle is the definition: a comparison sort on the pairs.
+ * ---------------------------------------------------------------------------------------- */
+typedef struct { uint32_t hash, id; } orc_pair;
+
+static int orc_pair_cmp(const void *a, const void *b)
+{
+    const orc_pair *p = (const orc_pair *)a, *q = (const orc_pair *)b;
+    if (p->hash != q->hash) return p->hash < q->hash ? -1 : 1;
+    if (p->id != q->id) return p->id < q->id ? -1 : 1;
+    return 0;
+}
+
+int orc_sort(int64_t n, const uint32_t *hash, uint32_t *sorted_hash, uint32_t *perm)
+{
+    orc_pair *p = (orc_pair *)malloc((size_t)(n > 0 ? n : 1) * sizeof(orc_pair));
+    if (!p) return -1;
+    for (int64_t i = 0; i < n; ++i) { p[i].hash = hash[i]; p[i].id = (uint32_t)i; }
+    qsort(p, (size_t)n, sizeof(orc_pair), orc_pair_cmp);
+    for (int64_t k = 0; k < n; ++k) { sorted_hash[k] = p[k].hash; perm[k] = p[k].id; }
+    free(p);
+    return 0;
+}
+
+/* ------------------------------------------------------------------------------------------
+ * O3  Cell start/end tables (BASELINE.json north_star: "with cell start/end tables"; implied by
+ * PAPER.md:13 "restricted to its bucket and to the surrounding buckets").  Reading S7:
+ * cell_start[c] = #{k : sorted_hash[k] <  c},  cell_end[c] = #{k : sorted_hash[k] <= c}.
+ * ---------------------------------------------------------------------------------------- */
+void orc_cell_ranges(int64_t n, const uint32_t *sorted_hash, int64_t n_cells, uint32_t *cell_start,
+                     uint32_t *cell_end)
+{
+    for (int64_t c = 0; c < n_cells; ++c) {
+        int64_t lo = 0, hi = n; /* first k with sorted_hash[k] >= c */
+        while (lo < hi) {
+            int64_t mid = lo + (hi - lo) / 2;
+            if ((int64_t)sorted_hash[mid] < c) lo = mid + 1; else hi = mid;
+        }
+        cell_start[c] = (uint32_t)lo;
+        hi = n;                 /* first k with sorted_hash[k] > c */
+        while (lo < hi) {
+            int64_t mid = lo + (hi - lo) / 2;
+            if ((int64_t)sorted_hash[mid] <= c) lo = mid + 1; else hi = mid;
+        }
+        cell_end[c] = (uint32_t)lo;
+    }
+}
+
+/* ------------------------------------------------------------------------------------------
+ * O4  Communication hash ("If particles from other GPUs are present in the
+ * particle's bucket or in the surrounding buckets, the communication hash number is equal to
+ * the hash number, otherwise it is equal to some garbage collector hash"; PAPER.md:22 step c).
+ * Plain per-particle definition.  Readings S9 (out-of-grid buckets skipped, no wrap), S10
+ * (bucket-level presence, not distance), S12 (every particle carries a label).
+ * All arrays are in sorted order (index k).
+ * ---------------------------------------------------------------------------------------- */
+void orc_comm_hash(int64_t n, const uint32_t *sorted_hash, const int32_t *sorted_owner,
+                   const int32_t *dims, const uint32_t *cell_start, const uint32_t *cell_end,
+                   uint32_t *comm_hash)
+{
+    const int64_t nx = dims[0], ny = dims[1], nz = dims[2];
+    for (int64_t k = 0; k < n; ++k) {
+        const int64_t hsh = sorted_hash[k];
+        const int64_t cx = hsh % nx, cy = (hsh / nx) % ny, cz = hsh / (nx * ny);
+        const int32_t o = sorted_owner[k];
+        int found = 0;
+        for (int64_t dz = -1; dz <= 1 && !found; ++dz)
+            for (int64_t dy = -1; dy <= 1 && !found; ++dy)
+                for (int64_t dx = -1; dx <= 1 && !found; ++dx) {
+                    const int64_t x = cx + dx, y = cy + dy, z = cz + dz;
+                    if (x < 0 || x >= nx || y < 0 || y >= ny || z < 0 || z >= nz) continue;
+                    const int64_t c = x + nx * (y + ny * z);
+                    for (uint32_t j = cell_start[c]; j < cell_end[c]; ++j)
+                        if (sorted_owner[j] != o) { found = 1; break; }
+                }
+        comm_hash[k] = found ? (uint32_t)hsh : ORC_GARBAGE;
+    }
+}
+
+/* ------------------------------------------------------------------------------------------
+ * O5  MGPU boundary particle set ("Then the particles can be sorted according to
+ * this communication hash, so that the data that shall be broadcasted to the other GPUs can be
+ * isolated").  The paper's algorithm is followed literally: a comparison sort of the particles
+ * on the key (comm_hash, id); the boundary list is the head of that order (everything before
+ * the first garbage key).  Reading S11: one global list plus per-owner counts.
+ * Returns the count M; boundary_ids has room for n entries.
+ * ---------------------------------------------------------------------------------------- */
+int64_t orc_boundary(int64_t n, const uint32_t *comm_hash, const uint32_t *perm,
+                     const int32_t *sorted_owner, int32_t n_owners, uint32_t *boundary_ids,
+                     uint32_t *owner_counts)
+{
+    orc_pair *p = (orc_pair *)malloc((size_t)(n > 0 ? n : 1) * sizeof(orc_pair));
+    int32_t *owner_of_id = (int32_t *)malloc((size_t)(n > 0 ? n : 1) * sizeof(int32_t));
+    if (!p || !owner_of_id) { free(p); free(owner_of_id); return -1; }
+    for (int64_t k = 0; k < n; ++k) {
+        p[k].hash = comm_hash[k];
+        p[k].id = perm[k];
+        owner_of_id[perm[k]] = sorted_owner[k];
+    }
+    qsort(p, (size_t)n, sizeof(orc_pair), orc_pair_cmp);
+    for (int32_t g = 0; g < n_owners; ++g) owner_counts[g] = 0;
+    int64_t m = 0;
+    while (m < n && p[m].hash != ORC_GARBAGE) {
+        boundary_ids[m] = p[m].id;
+        owner_counts[owner_of_id[p[m].id]] += 1;
+        ++m;
+    }
+    free(p);
+    free(owner_of_id);
+    return m;
+}
+
+/* ------------------------------------------------------------------------------------------
+ * O6  Kernel (BASELINE.json configs[0]: "Wendland C2 kernel with support 2h"; reading S14).
+ * q = r/h;  W = alpha (1 - q/2)^4 (1 + 2q),  alpha = 21 / (16 pi h^3)   for q < 2, else 0.
+ * grad_i W_ij = F(r) x_ij with F(r) = (dW/dr)/r = -(5 alpha / h^2) (1 - q/2)^3.
+ * ---------------------------------------------------------------------------------------- */
+double orc_kernel_W(double r, double h)
+{
+    const double q = r / h;
+    if (q >= 2.0) return 0.0;
+    const double alpha = 21.0 / (16.0 * M_PI * h * h * h);
+    const double t = 1.0 - 0.5 * q;
+    return alpha * t * t * t * t * (1.0 + 2.0 * q);
+}
+
+double orc_kernel_F(double r, double h)
+{
+    const double q = r / h;
+    if (q >= 2.0) return 0.0;
+    const double alpha = 21.0 / (16.0 * M_PI * h * h * h);
+    const double t = 1.0 - 0.5 * q;
+    return -(5.0 * alpha / (h * h)) * t * t * t;
+}
+
+/* ------------------------------------------------------------------------------------------
+ * O7 + O8  Interaction loops and stress rate (PAPER.md:13 neighbour search in own + surrounding
+ * buckets; PAPER.md:24-25 steps e, f; "several interaction loops for one iteration";
+ * BASELINE.json north_star: "density rate and momentum/stress divergence").  Readings S13-S19.
+ *
+ * Neighbours of i: every j != i in the 27-bucket stencil of i's bucket (out-of-grid buckets
+ * skipped) with r_ij^2 < (2h)^2, compared in fp64 on the widened fp32 positions.
+ *   loop 1:  Drho_i   = sum_j m_j (v_i - v_j) . grad_i W_ij
+ *            L_i[a][b] = sum_j (m_j / rho_j) (v_j - v_i)_a (grad_i W_ij)_b
+ *   loop 2:  a_i      = sum_j m_j (sigma_i/rho_i^2 + sigma_j/rho_j^2) . grad_i W_ij
+ *   O8:      D = (L + L^T)/2, Om = (L - L^T)/2,
+ *            dsig = K tr(D) I + 2G (D - tr(D)/3 I) + Om sigma - sigma Om
+ *
+ * All arrays are in sorted order.  posm [n][4] = x,y,z,m; velr [n][4] = vx,vy,vz,rho;
+ * sig [6][n] = xx,yy,zz,xy,xz,yz.  If idx != NULL only the n_idx particles idx[] are computed
+ * and outputs are indexed by position in idx (used for sampled parity at full size).
+ * Outputs: drho[m], L[m][9] (row major a,b), acc[m][3], dsig[m][6]; *pair_count = number of
+ * ordered accepted pairs (S25).
+ * ---------------------------------------------------------------------------------------- */
+static void orc_sym_load(const float *sig, int64_t n, int64_t k, double s[3][3])
+{
+    const double xx = sig[0 * n + k], yy = sig[1 * n + k], zz = sig[2 * n + k];
+    const double xy = sig[3 * n + k], xz = sig[4 * n + k], yz = sig[5 * n + k];
+    s[0][0] = xx; s[1][1] = yy; s[2][2] = zz;
+    s[0][1] = s[1][0] = xy;
+    s[0][2] = s[2][0] = xz;
+    s[1][2] = s[2][1] = yz;
+}
+
+void orc_interact(int64_t n, const float *posm, const float *velr, const float *sig,
+                  const uint32_t *sorted_hash, const int32_t *dims, const uint32_t *cell_start,
+                  const uint32_t *cell_end, float h_f32, float K_f32, float G_f32,
+                  int64_t n_idx, const int64_t *idx,
+                  double *drho, double *L, double *acc, double *dsig, int64_t *pair_count)
+{
+    const double h = (double)h_f32, K = (double)K_f32, G = (double)G_f32;
+    const double support2 = (2.0 * h) * (2.0 * h);
+    const int64_t nx = dims[0], ny = dims[1], nz = dims[2];
+    const int64_t m_out = idx ? n_idx : n;
+    int64_t pairs = 0;
+
+    for (int64_t out = 0; out < m_out; ++out) {
+        const int64_t i = idx ? idx[out] : out;
+        const int64_t hsh = sorted_hash[i];
+        const int64_t cx = hsh % nx, cy = (hsh / nx) % ny, cz = hsh / (nx * ny);
+        const double xi[3] = { posm[4 * i + 0], posm[4 * i + 1], posm[4 * i + 2] };
+        const double vi[3] = { velr[4 * i + 0], velr[4 * i + 1], velr[4 * i + 2] };
+        const double rhoi = velr[4 * i + 3];
+        double si[3][3];
+        orc_sym_load(sig, n, i, si);
+
+        /* ---- loop 1: density rate and velocity gradient ---- */
+        double dr = 0.0, Li[3][3] = { { 0 } };
+        for (int64_t dz = -1; dz <= 1; ++dz)
+            for (int64_t dy = -1; dy <= 1; ++dy)
+                for (int64_t dx = -1; dx <= 1; ++dx) {
+                    const int64_t x = cx + dx, y = cy + dy, z = cz + dz;
+                    if (x < 0 || x >= nx || y < 0 || y >= ny || z < 0 || z >= nz) continue;
+                    const int64_t c = x + nx * (y + ny * z);
+                    for (int64_t j = cell_start[c]; j < (int64_t)cell_end[c]; ++j) {
+                        if (j == i) continue; /* S15 */
+                        const double xij[3] = { xi[0] - posm[4 * j + 0], xi[1] - posm[4 * j + 1],
+                                                xi[2] - posm[4 * j + 2] };
+                        const double r2 = xij[0] * xij[0] + xij[1] * xij[1] + xij[2] * xij[2];
+                        if (!(r2 < support2)) continue;
+                        ++pairs;
+                        const double F = orc_kernel_F(sqrt(r2), h);
+                        const double mj = posm[4 * j + 3], rhoj = velr[4 * j + 3];
+                        const double gW[3] = { F * xij[0], F * xij[1], F * xij[2] };
+                        const double vij[3] = { vi[0] - velr[4 * j + 0], vi[1] - velr[4 * j + 1],
+                                                vi[2] - velr[4 * j + 2] };
+                        dr += mj * (vij[0] * gW[0] + vij[1] * gW[1] + vij[2] * gW[2]);
+                        for (int a = 0; a < 3; ++a)
+                            for (int b = 0; b < 3; ++b)
+                                Li[a][b] += (mj / rhoj) * (-vij[a]) * gW[b];
+                    }
+                }
+
+        /* ---- loop 2: momentum (stress divergence) ---- */
+        double ai[3] = { 0, 0, 0 };
+        for (int64_t dz = -1; dz <= 1; ++dz)
+            for (int64_t dy = -1; dy <= 1; ++dy)
+                for (int64_t dx = -1; dx <= 1; ++dx) {
+                    const int64_t x = cx + dx, y = cy + dy, z = cz + dz;
+                    if (x < 0 || x >= nx || y < 0 || y >= ny || z < 0 || z >= nz) continue;
+                    const int64_t c = x + nx * (y + ny * z);
+                    for (int64_t j = cell_start[c]; j < (int64_t)cell_end[c]; ++j) {
+                        if (j == i) continue;
+                        const double xij[3] = { xi[0] - posm[4 * j + 0], xi[1] - posm[4 * j + 1],
+                                                xi[2] - posm[4 * j + 2] };
+                        const double r2 = xij[0] * xij[0] + xij[1] * xij[1] + xij[2] * xij[2];
+                        if (!(r2 < support2)) continue;
+                        const double F = orc_kernel_F(sqrt(r2), h);
+                        const double mj = posm[4 * j + 3], rhoj = velr[4 * j + 3];
+                        double sj[3][3];
+                        orc_sym_load(sig, n, j, sj);
+                        for (int a = 0; a < 3; ++a) {
+                            double t = 0.0;
+                            for (int b = 0; b < 3; ++b)
+                                t += (si[a][b] / (rhoi * rhoi) + sj[a][b] / (rhoj * rhoj)) *
+                                     (F * xij[b]);
+                            ai[a] += mj * t;
+                        }
+                    }
+                }
+
+        /* ---- O8: Hooke's law in rate form with the Jaumann rate ---- */
+        double D[3][3], Om[3][3];
+        for (int a = 0; a < 3; ++a)
+            for (int b = 0; b < 3; ++b) {
+                D[a][b] = 0.5 * (Li[a][b] + Li[b][a]);
+                Om[a][b] = 0.5 * (Li[a][b] - Li[b][a]);
+            }
+        const double trD = D[0][0] + D[1][1] + D[2][2];
+        double sd[3][3];
+        for (int a = 0; a < 3; ++a)
+            for (int b = 0; b < 3; ++b) {
+                double v = 2.0 * G * (D[a][b] - (a == b ? trD / 3.0 : 0.0)) +
+                           (a == b ? K * trD : 0.0);
+                for (int c = 0; c < 3; ++c) v += Om[a][c] * si[c][b] - si[a][c] * Om[c][b];
+                sd[a][b] = v;
+            }
+
+        drho[out] = dr;
+        for (int a = 0; a < 3; ++a) {
+            acc[3 * out + a] = ai[a];
+            for (int b = 0; b < 3; ++b) L[9 * out + 3 * a + b] = Li[a][b];
+        }
+        dsig[6 * out + 0] = sd[0][0]; dsig[6 * out + 1] = sd[1][1]; dsig[6 * out + 2] = sd[2][2];
+        dsig[6 * out + 3] = sd[0][1]; dsig[6 * out + 4] = sd[0][2]; dsig[6 * out + 5] = sd[1][2];
+    }
+    if (pair_count) *pair_count = pairs;
+}
+
+/* ------------------------------------------------------------------------------------------
+ * O9  Explicit integration (PAPER.md:26 step g: "Each GPU can integrate its equations").
+ * Reading S18: symplectic Euler.  rho+ = rho + dt Drho; v+ = v + dt a; sigma+ = sigma + dt dsig;
+ * x+ = x + dt v+.  Mass unchanged.  Inputs fp32 state + fp64 rates (layouts as orc_interact's
+ * outputs); outputs fp64: posm_out [n][4], velr_out [n][4], sig_out [6][n].
+ * ---------------------------------------------------------------------------------------- */
+void orc_integrate(int64_t n, double dt, const float *posm, const float *velr, const float *sig,
+                   const double *drho, const double *acc, const double *dsig, double *posm_out,
+                   double *velr_out, double *sig_out)
+{
+    for (int64_t i = 0; i < n; ++i) {
+        double vp[3];
+        for (int a = 0; a < 3; ++a) {
+            vp[a] = (double)velr[4 * i + a] + dt * acc[3 * i + a];
+            velr_out[4 * i + a] = vp[a];
+            posm_out[4 * i + a] = (double)posm[4 * i + a] + dt * vp[a];
+        }
+        posm_out[4 * i + 3] = (double)posm[4 * i + 3];
+        velr_out[4 * i + 3] = (double)velr[4 * i + 3] + dt * drho[i];
+        for (int c = 0; c < 6; ++c)
+            sig_out[(int64_t)c * n + i] = (double)sig[(int64_t)c * n + i] + dt * dsig[6 * i + c];
+    }
+}

@@ -1,0 +1,457 @@
+"""Pins for the CPU oracle (oracle/sph_oracle.c) -- everything here runs without a GPU.
+
+The oracle is pinned to things other than itself: brute-force O(N^2) enumeration written with
+dense numpy (no buckets), library routines (numpy.lexsort / searchsorted, scipy quad / expm),
+closed forms and invariants (I0-I10), and the lattice constants in
+tests/golden/lattice_closed_forms.txt.
+"""
+import os
+
+import numpy as np
+import pytest
+from scipy.integrate import quad
+from scipy.linalg import expm
+
+import oracle as orc
+from paper_2310_03596_b200 import workloads as W
+
+GOLDEN = os.path.join(os.path.dirname(__file__), "golden")
+H = float(np.float32(1.3))
+
+
+# ----------------------------------------------------------------------------- helpers
+def bucket_coords_f32(posm, origin, dims, h):
+    """numpy-float32 emulation of the pinned fp32 sequence (reading S2)."""
+    edge = np.float32(2.0) * np.float32(h)
+    inv = np.float32(1.0) / edge
+    t = posm[:, :3].astype(np.float32) - origin.astype(np.float32)[None, :]
+    u = (t * inv).astype(np.float32)
+    f = np.floor(u)
+    f = np.clip(f, 0, (dims - 1)[None, :].astype(np.float32))
+    return f.astype(np.int64)
+
+
+def sym6_to_mat(s6):
+    xx, yy, zz, xy, xz, yz = s6
+    return np.array([[xx, xy, xz], [xy, yy, yz], [xz, yz, zz]])
+
+
+def brute_force_rates(posm, velr, sig, h, K, G):
+    """Dense O(N^2) evaluation; neighbours by distance only (I0)."""
+    x = posm[:, :3].astype(np.float64); m = posm[:, 3].astype(np.float64)
+    v = velr[:, :3].astype(np.float64); rho = velr[:, 3].astype(np.float64)
+    n = x.shape[0]
+    S = np.zeros((n, 3, 3))
+    for k, (a, b) in enumerate([(0, 0), (1, 1), (2, 2), (0, 1), (0, 2), (1, 2)]):
+        S[:, a, b] = sig[k]; S[:, b, a] = sig[k]
+    xij = x[:, None, :] - x[None, :, :]
+    r = np.sqrt((xij ** 2).sum(-1))
+    nb = (r < 2 * h) & ~np.eye(n, dtype=bool)
+    alpha = 21.0 / (16.0 * np.pi * h ** 3)
+    # dW/dr from the closed form of W, differentiated by hand independently of orc_kernel_F:
+    # W = alpha (1-q/2)^4 (1+2q)  =>  dW/dq = -5 alpha q (1-q/2)^3
+    q = r / h
+    dWdr = np.where(nb, -5.0 * alpha * q * (1 - q / 2) ** 3 / h, 0.0)
+    with np.errstate(invalid="ignore", divide="ignore"):
+        e = np.where(r[..., None] > 0, xij / r[..., None], 0.0)
+    gW = dWdr[..., None] * e                      # grad_i W_ij
+    vij = v[:, None, :] - v[None, :, :]
+    drho = (m[None, :] * (vij * gW).sum(-1)).sum(1)
+    L = np.einsum("j,ija,ijb->iab", m / rho, -vij, gW) if False else \
+        np.einsum("ij,ija,ijb->iab", np.broadcast_to((m / rho)[None, :], (n, n)), -vij, gW)
+    Sr = S / (rho ** 2)[:, None, None]
+    acc = np.einsum("j,ijab,ijb->ia", m, Sr[:, None] + Sr[None, :], gW)
+    D = 0.5 * (L + L.transpose(0, 2, 1)); Om = 0.5 * (L - L.transpose(0, 2, 1))
+    trD = np.trace(D, axis1=1, axis2=2)
+    I = np.eye(3)
+    sd = K * trD[:, None, None] * I + 2 * G * (D - trD[:, None, None] / 3 * I) + Om @ S - S @ Om
+    dsig = np.stack([sd[:, 0, 0], sd[:, 1, 1], sd[:, 2, 2], sd[:, 0, 1], sd[:, 0, 2], sd[:, 1, 2]], 1)
+    return drho, L, acc, dsig, int(nb.sum())
+
+
+def sorted_view(w):
+    r = orc.step(w.posm, w.velr, w.sig, w.owner, w.origin, w.dims, w.h, w.K, w.G, w.n_owners,
+                 w.dt, floats=False)
+    p = r.perm
+    return r, w.posm[p], w.velr[p], np.ascontiguousarray(w.sig[:, p]), w.owner[p]
+
+
+def rates_of(w):
+    r, sp, sv, ss, so = sorted_view(w)
+    return r, orc.interact(sp, sv, ss, r.sorted_hash, w.dims, r.cell_start, r.cell_end, w.h, w.K, w.G), \
+        (sp, sv, ss, so)
+
+
+def custom_block(spacing, side, h, vel_fn=None, sig_fn=None, rho=1.0):
+    """Un-jittered lattice with arbitrary spacing (continuum-limit pins)."""
+    g = np.arange(side) * spacing
+    X, Y, Z = np.meshgrid(g, g, g, indexing="ij")
+    x = np.stack([X.ravel(), Y.ravel(), Z.ravel()], 1)
+    n = x.shape[0]
+    posm = np.empty((n, 4), np.float32); posm[:, :3] = x; posm[:, 3] = rho * spacing ** 3
+    velr = np.zeros((n, 4), np.float32); velr[:, 3] = rho
+    if vel_fn is not None:
+        velr[:, :3] = vel_fn(x)
+    sig = np.zeros((6, n), np.float32)
+    if sig_fn is not None:
+        sig[:] = sig_fn(x)
+    origin, dims = W.grid_for((g[-1],) * 3, h)
+    return W.Workload("custom", posm, velr, sig, np.zeros(n, np.int32), origin, dims,
+                      h=np.float32(h))
+
+
+def interior_index(w, sp):
+    c = sp[:, :3].astype(np.float64)
+    centre = 0.5 * (c.max(0) + c.min(0))
+    return int(np.argmin(((c - centre) ** 2).sum(1)))
+
+
+# ----------------------------------------------------------------------------- O1 hash
+def test_hash_fp32_sequence_faces_and_clamp():
+    origin, dims = W.grid_for((15, 15, 15))
+    edge = np.float32(2.0) * np.float32(H)
+    pts = []
+    for k in range(0, 8):
+        face = np.float32(origin[0] + np.float32(k) * edge)
+        for d in (-2, -1, 0, 1, 2):
+            x = face
+            for _ in range(abs(d)):
+                x = np.nextafter(x, np.float32(np.inf if d > 0 else -np.inf), dtype=np.float32)
+            pts.append([x, 0.0, 0.0, 1.0])
+    pts += [[-1e6, 3.0, 3.0, 1.0], [1e6, 1e7, -1e9, 1.0], [3e38, -3e38, 0.0, 1.0]]
+    posm = np.array(pts, np.float32)
+    got = orc.hash(posm, origin, dims, H)
+    c = bucket_coords_f32(posm, origin, dims, H)
+    exp = c[:, 0] + dims[0] * (c[:, 1] + dims[1] * c[:, 2])
+    assert np.array_equal(got, exp.astype(np.uint32))
+    # clamping (S3): far outside -> border buckets
+    assert got[-3] == 0 + dims[0] * (c[-3, 1] + dims[1] * c[-3, 2]) and c[-3, 0] == 0
+    assert tuple(c[-2]) == (dims[0] - 1, dims[1] - 1, 0)
+    assert tuple(c[-1]) == (dims[0] - 1, 0, 1)       # z = 0 - (-2.6) = 2.6 -> bucket 0 or 1
+    # monotone in x
+    xs = np.sort(np.random.default_rng(0).uniform(-5, 25, 2000).astype(np.float32))
+    pm = np.zeros((2000, 4), np.float32); pm[:, 0] = xs
+    hx = orc.hash(pm, origin, dims, H).astype(np.int64)
+    # y = z = 0 -> bucket (cx, 1, 1) since 0 - (-2.6) = 2.6 = one edge (up to rounding)
+    assert np.all(np.diff(hx) >= 0)
+
+
+def test_hash_bijection_bucket_centres():
+    """S1: linear, x fastest -- every bucket gets its own hash, decodable."""
+    dims = np.array([5, 4, 3], np.int32)
+    origin = np.array([-1.0, 2.0, 0.5], np.float32)
+    edge = 2 * H
+    cz, cy, cx = np.meshgrid(np.arange(3), np.arange(4), np.arange(5), indexing="ij")
+    posm = np.zeros((60, 4), np.float32)
+    posm[:, 0] = origin[0] + (cx.ravel() + 0.5) * edge
+    posm[:, 1] = origin[1] + (cy.ravel() + 0.5) * edge
+    posm[:, 2] = origin[2] + (cz.ravel() + 0.5) * edge
+    got = orc.hash(posm, origin, dims, H)
+    assert np.array_equal(got, np.arange(60, dtype=np.uint32))   # enumeration order = x fastest
+
+
+# ----------------------------------------------------------------------------- O2 sort
+@pytest.mark.parametrize("n,nkeys", [(0, 4), (1, 4), (1000, 7), (50000, 100000), (4096, 1)])
+def test_sort_vs_lexsort(n, nkeys):
+    rng = np.random.default_rng(n + nkeys)
+    h = rng.integers(0, nkeys, n).astype(np.uint32)
+    sh, perm = orc.sort(h)
+    exp = np.lexsort((np.arange(n), h))
+    assert np.array_equal(perm, exp.astype(np.uint32))
+    assert np.array_equal(sh, h[exp])
+
+
+# ----------------------------------------------------------------------------- O3 cell tables
+def test_cell_ranges_vs_searchsorted_and_identities():
+    rng = np.random.default_rng(3)
+    C = 300
+    h = np.sort(rng.choice(np.arange(5, 290), 2000)).astype(np.uint32)    # empty head/tail/gaps
+    cs, ce = orc.cell_ranges(h, C)
+    assert np.array_equal(cs, np.searchsorted(h, np.arange(C), "left"))
+    assert np.array_equal(ce, np.searchsorted(h, np.arange(C), "right"))
+    assert cs[0] == 0 and ce[-1] == 2000 and np.array_equal(ce[:-1], cs[1:])
+    assert int((ce.astype(np.int64) - cs).sum()) == 2000
+    cs0, ce0 = orc.cell_ranges(np.zeros(0, np.uint32), 7)
+    assert not cs0.any() and not ce0.any()
+
+
+# ----------------------------------------------------------------------------- O4/O5 comm hash
+def brute_comm_flags(posm, owner, origin, dims, h):
+    c = bucket_coords_f32(posm, origin, dims, h)
+    near = (np.abs(c[:, None, :] - c[None, :, :]) <= 1).all(-1)
+    other = owner[:, None] != owner[None, :]
+    return (near & other).any(1)
+
+
+@pytest.mark.parametrize("owners", [("plane_x", 5.0), ("random", 16), ("single",), ("slabs", 3),
+                                    ("slabs_mixed", 4, 0.02)])
+def test_comm_hash_and_boundary_bruteforce(owners):
+    w = W.lattice_block(11, 9, 10, 0.1, 77, owners=owners)
+    r, sp, sv, ss, so = sorted_view(w)
+    flags = brute_comm_flags(w.posm, w.owner, w.origin, w.dims, w.h)       # id order
+    exp_comm = np.where(flags[r.perm], r.sorted_hash, np.uint32(orc.GARBAGE))
+    assert np.array_equal(r.comm_hash, exp_comm)
+    # I6: head of the sort on comm hash == stable compaction of the (hash,id)-sorted array
+    assert np.array_equal(r.boundary_ids, r.perm[flags[r.perm]])
+    assert np.array_equal(r.owner_counts, np.bincount(w.owner[r.boundary_ids], minlength=w.n_owners))
+    # I5: the flag is a per-bucket property
+    for c in np.unique(r.sorted_hash):
+        f = r.comm_hash[r.sorted_hash == c] != orc.GARBAGE
+        assert f.all() or not f.any()
+    # I4 completeness: every pair r<2h with different owners has both ends in the set
+    x = w.posm[:, :3].astype(np.float64)
+    d2 = ((x[:, None] - x[None]) ** 2).sum(-1)
+    pair = (d2 < (2 * H) ** 2) & (w.owner[:, None] != w.owner[None, :])
+    inset = np.zeros(w.n, bool); inset[r.boundary_ids] = True
+    ii, jj = np.nonzero(pair)
+    assert inset[ii].all() and inset[jj].all()
+    if owners[0] == "single":
+        assert r.boundary_ids.size == 0                   # I10 / S12
+    if owners[0] == "random":
+        assert r.boundary_ids.size == w.n                 # PAPER.md:30 full mixing
+
+
+def test_boundary_slabs_lie_on_surfaces():
+    """with slabs the MGPU boundary particles lie 'onto two surfaces'."""
+    w = W.lattice_block(40, 8, 8, 0.1, 5, owners=("slabs", 3))
+    r, *_ = sorted_view(w)
+    xb = w.posm[r.boundary_ids, 0]
+    interfaces = np.array([40 / 3 - 0.5, 80 / 3 - 0.5])
+    dist = np.abs(xb[:, None] - interfaces[None, :]).min(1)
+    assert dist.max() <= 2 * 2 * H + 0.2                   # within two bucket layers
+    assert 0 < r.boundary_ids.size < w.n // 2
+
+
+# ----------------------------------------------------------------------------- O6 kernel
+def test_kernel_normalisation_and_gradient():
+    for h in (0.7, H, 2.0):
+        val, err = quad(lambda r: 4 * np.pi * r * r * orc.kernel_W(r, h), 0, 2 * h, epsabs=1e-13)
+        assert abs(val - 1.0) < 1e-10                                       # I1
+        assert orc.kernel_W(2 * h, h) == 0.0 and orc.kernel_F(2 * h, h) == 0.0
+        assert orc.kernel_W(2.5 * h, h) == 0.0
+        for r in np.linspace(0.05 * h, 1.95 * h, 23):
+            e = 1e-6 * h
+            dW = (orc.kernel_W(r + e, h) - orc.kernel_W(r - e, h)) / (2 * e)
+            assert abs(orc.kernel_F(r, h) * r - dW) < 1e-8 * abs(orc.kernel_W(0, h)) / h
+        assert orc.kernel_F(0.3 * h, h) < 0                                  # W decreasing
+    # alpha(h=1.3) from SURVEY.md I1
+    assert abs(orc.kernel_W(0.0, 1.3) - 0.19016009359) < 1e-10
+
+
+# ----------------------------------------------------------------------------- O7/O8 vs brute force
+@pytest.mark.parametrize("make", [lambda: W.t1b(10, 1100), lambda: W.t1b(12, 1101),
+                                  lambda: W.config(1, side=12)])
+def test_interact_vs_bruteforce(make):
+    w = make()
+    r, rt, (sp, sv, ss, so) = rates_of(w)
+    drho, L, acc, dsig, pairs = brute_force_rates(sp, sv, ss, float(w.h), float(w.K), float(w.G))
+    assert rt.pair_count == pairs
+    for got, exp in ((rt.drho, drho), (rt.L, L), (rt.acc, acc), (rt.dsig, dsig)):
+        scale = max(np.abs(exp).max(), 1e-300)
+        assert np.abs(got - exp).max() <= 1e-11 * scale
+
+
+def test_interact_subset_matches_full():
+    w = W.t1b(10, 1102)
+    r, rt, (sp, sv, ss, so) = rates_of(w)
+    idx = np.array([0, 5, 17, 400, 999], np.int64)
+    sub = orc.interact(sp, sv, ss, r.sorted_hash, w.dims, r.cell_start, r.cell_end, w.h, w.K, w.G,
+                       idx=idx)
+    assert np.array_equal(sub.drho, rt.drho[idx]) and np.array_equal(sub.acc, rt.acc[idx])
+    assert np.array_equal(sub.dsig, rt.dsig[idx]) and np.array_equal(sub.L, rt.L[idx])
+
+
+def test_momentum_conservation():
+    """I2: symmetric pair forces => sum_i m_i a_i = 0 to rounding."""
+    w = W.t1b(12, 1103)
+    w.posm[:, 3] = (1.0 + 0.2 * np.random.default_rng(1).random(w.n)).astype(np.float32)
+    r, rt, (sp, *_ ) = rates_of(w)
+    f = sp[:, 3:4].astype(np.float64) * rt.acc
+    assert np.abs(f.sum(0)).max() <= 1e-12 * np.abs(f).sum()
+    assert np.abs(f).sum() > 0
+
+
+def test_uniform_translation_gives_exact_zero():
+    """I3: uniform v => Drho == 0 and L == 0 exactly, any geometry (incl. free surfaces)."""
+    w = W.t1b(10, 1104)
+    w.velr[:, :3] = np.array([0.3, -1.7, 2.2], np.float32)
+    r, rt, _ = rates_of(w)
+    assert not rt.drho.any() and not rt.L.any()
+    assert np.abs(rt.acc).max() > 0          # stress still acts
+
+
+def test_rest_lattice_all_zero():
+    w = W.config(0, side=8)
+    r, rt, _ = rates_of(w)
+    assert not rt.drho.any() and not rt.acc.any() and not rt.dsig.any()
+    assert rt.pair_count > 0
+
+
+def test_uniform_density_continuity_identity():
+    """I7: uniform rho and m  =>  Drho_i = -rho tr(L_i)."""
+    w = W.config(4, side=10)
+    r, rt, _ = rates_of(w)
+    tr = np.trace(rt.L, axis1=1, axis2=2)
+    assert np.abs(rt.drho + 1.0 * tr).max() <= 1e-13 * np.abs(rt.drho).max()
+
+
+def test_lattice_closed_forms_golden():
+    """I8 / tests/golden/lattice_closed_forms.txt (unit lattice, h = 1.3, interior particle)."""
+    gold = {}
+    for line in open(os.path.join(GOLDEN, "lattice_closed_forms.txt")):
+        if line.strip() and not line.startswith("#"):
+            k, v = line.split()[:2]
+            gold[k] = float(v)
+    A = np.array([[0.0, 0.0, 0.0], [0.0, 0.0, 0.0], [0.0, 0.0, -0.001]])
+    w = custom_block(1.0, 9, H, vel_fn=lambda x: x @ A.T)
+    r, rt, (sp, *_ ) = rates_of(w)
+    i = interior_index(w, sp)
+    sub = orc.interact(sp, w.velr[r.perm], np.ascontiguousarray(w.sig[:, r.perm]), r.sorted_hash,
+                       w.dims, r.cell_start, r.cell_end, w.h, w.K, w.G, idx=np.array([i]))
+    assert sub.pair_count == int(gold["neighbours"])
+    # geometry-only count: lattice points with 0 < |p| < 2.6
+    g = np.arange(-3, 4)
+    P = np.stack(np.meshgrid(g, g, g, indexing="ij"), -1).reshape(-1, 3)
+    assert int(((P ** 2).sum(1) < 2.6 ** 2).sum()) - 1 == int(gold["neighbours"])
+    sumW = sum(orc.kernel_W(float(np.sqrt(p @ p)), 1.3) for p in P)
+    assert abs(sumW - gold["sum_W_incl_self"]) < 2e-9
+    assert abs(rt.L[i, 2, 2] / A[2, 2] - gold["moment_M"]) < 2e-6      # fp32 positions/velocities
+    assert abs(rt.drho[i] / 0.001 - gold["moment_M"]) < 2e-6
+
+
+# ----------------------------------------------------------------------------- continuum limits
+def test_continuum_velocity_gradient_sign_and_index():
+    """Dense lattice (h/dx = 2.6): L -> grad v with L[a][b] = dv_a/dx_b, Drho -> -rho div v."""
+    A = np.array([[0.010, 0.020, -0.005], [0.000, -0.030, 0.015], [0.025, -0.010, 0.004]])
+    rho = 1.7
+    w = custom_block(0.5, 23, H, vel_fn=lambda x: x @ A.T, rho=rho)
+    r, sp, sv, ss, so = sorted_view(w)
+    i = interior_index(w, sp)
+    sub = orc.interact(sp, sv, ss, r.sorted_hash, w.dims, r.cell_start, r.cell_end, w.h, w.K, w.G,
+                       idx=np.array([i]))
+    assert np.abs(sub.L[0] - A).max() < 2e-3 * np.abs(A).max()
+    assert abs(sub.drho[0] + rho * np.trace(A)) < 2e-3 * rho * np.abs(A).max()
+
+
+def test_continuum_stress_divergence_sign_and_index():
+    """a_a -> (1/rho) d sigma_ab / d x_b for a linear stress field (tension positive)."""
+    rng = np.random.default_rng(11)
+    B = rng.normal(size=(6, 3)) * 1e-3                  # d sig6 / d x
+    s0 = rng.normal(size=6) * 1e-2
+    rho = 0.8
+
+    def sig_fn(x):
+        return (s0[:, None] + B @ x.T)
+
+    w = custom_block(0.5, 23, H, sig_fn=sig_fn, rho=rho)
+    r, sp, sv, ss, so = sorted_view(w)
+    i = interior_index(w, sp)
+    sub = orc.interact(sp, sv, ss, r.sorted_hash, w.dims, r.cell_start, r.cell_end, w.h, w.K, w.G,
+                       idx=np.array([i]))
+    # div: a_x = d sxx/dx + d sxy/dy + d sxz/dz ; components xx,yy,zz,xy,xz,yz = 0..5
+    div = np.array([B[0, 0] + B[3, 1] + B[4, 2], B[3, 0] + B[1, 1] + B[5, 2],
+                    B[4, 0] + B[5, 1] + B[2, 2]]) / rho
+    assert np.abs(sub.acc[0] - div).max() < 3e-3 * np.abs(div).max()
+
+
+# ----------------------------------------------------------------------------- O8 textbook cases
+def lattice_L_factor():
+    A = np.diag([1e-3, 0.0, 0.0])
+    w = custom_block(1.0, 9, H, vel_fn=lambda x: x @ A.T)
+    r, rt, (sp, *_ ) = rates_of(w)
+    return rt.L[interior_index(w, sp), 0, 0] / 1e-3
+
+
+def stress_rate_for(A, s6, K=1.0, G=0.5):
+    w = custom_block(1.0, 9, H, vel_fn=lambda x: x @ A.T,
+                     sig_fn=lambda x: np.repeat(np.asarray(s6)[:, None], x.shape[0], 1))
+    w.K, w.G = np.float32(K), np.float32(G)
+    r, rt, (sp, *_ ) = rates_of(w)
+    i = interior_index(w, sp)
+    return rt.dsig[i], rt.L[i]
+
+
+def test_stress_rate_textbook_cases():
+    ms = lattice_L_factor()
+    eps, gam = 2e-3, 3e-3
+    # pure dilation: sigma_dot = K * 3 eps * I  (bulk modulus definition)
+    d, L = stress_rate_for(np.eye(3) * eps, np.zeros(6), K=2.0, G=0.7)
+    assert np.allclose(d, [3 * 2.0 * eps * ms] * 3 + [0, 0, 0], rtol=2e-6, atol=1e-12)
+    # simple shear v_x = gam*y: sigma_xy_dot = G*gam, no normal stress rate without pre-stress
+    A = np.zeros((3, 3)); A[0, 1] = gam
+    d, L = stress_rate_for(A, np.zeros(6), K=2.0, G=0.7)
+    assert np.allclose(d, [0, 0, 0, 0.7 * gam * ms, 0, 0], rtol=2e-6, atol=1e-12)
+    # uniaxial strain: sigma_xx_dot = (K + 4G/3) eps ; sigma_yy_dot = (K - 2G/3) eps
+    d, L = stress_rate_for(np.diag([eps, 0, 0]), np.zeros(6), K=2.0, G=0.7)
+    assert np.allclose(d, [(2.0 + 4 * 0.7 / 3) * eps * ms, (2.0 - 2 * 0.7 / 3) * eps * ms,
+                           (2.0 - 2 * 0.7 / 3) * eps * ms, 0, 0, 0], rtol=2e-6, atol=1e-12)
+
+
+def test_jaumann_rate_is_finite_rotation_derivative():
+    """S17: rigid spin of a pre-stressed body: sigma(t) = R sigma R^T, R = expm(Om t)."""
+    ms = lattice_L_factor()
+    Om = np.array([[0, -2e-3, 1e-3], [2e-3, 0, 3e-3], [-1e-3, -3e-3, 0]])
+    s6 = np.array([0.02, -0.01, 0.005, 0.004, -0.003, 0.006])
+    d, L = stress_rate_for(Om, s6)
+    S = sym6_to_mat(s6)
+    t = 1e-3
+    Rp, Rm = expm(ms * Om * t), expm(-ms * Om * t)
+    fd = (Rp @ S @ Rp.T - Rm @ S @ Rm.T) / (2 * t)
+    got = sym6_to_mat(d)
+    assert np.abs(got - fd).max() < 2e-5 * np.abs(fd).max()     # inputs are rounded to fp32
+    assert abs(np.trace(got)) < 1e-5 * np.abs(got).max()          # tr(sigma) invariant
+    assert abs((S * got).sum()) < 1e-5 * np.abs(S).max() * np.abs(got).max()  # sigma:sigma invariant
+
+
+# ----------------------------------------------------------------------------- misc readings
+def test_coincident_particles_no_nan():
+    """S15: distinct coincident particles are a pair with grad W = 0."""
+    w = W.t1b(6, 1105)
+    w.posm[1, :3] = w.posm[0, :3]
+    r, rt, _ = rates_of(w)
+    for a in (rt.drho, rt.L, rt.acc, rt.dsig):
+        assert np.isfinite(a).all()
+
+
+def test_integrate_symplectic_euler_by_hand():
+    n = 3
+    posm = np.array([[1, 2, 3, 1.5]] * n, np.float32)
+    velr = np.array([[0.1, -0.2, 0.3, 2.0]] * n, np.float32)
+    sig = np.arange(18, dtype=np.float32).reshape(6, n) * 0.01
+    drho = np.array([0.5, -0.5, 0.0]); acc = np.array([[1.0, 2.0, -3.0]] * n)
+    dsig = np.arange(18, dtype=np.float64).reshape(n, 6)
+    dt = 0.25
+    po, vo, so = orc.integrate(dt, posm, velr, sig, drho, acc, dsig)
+    vexp = velr[0, :3].astype(np.float64) + dt * acc[0]
+    assert np.allclose(vo[0, :3], vexp, rtol=0, atol=1e-15)
+    assert np.allclose(po[0, :3], posm[0, :3].astype(np.float64) + dt * vexp, rtol=0, atol=1e-15)  # uses v+
+    assert po[0, 3] == 1.5 and np.allclose(vo[:, 3], 2.0 + dt * drho)
+    assert np.allclose(so, sig.astype(np.float64) + dt * dsig.T)
+    po0, vo0, so0 = orc.integrate(0.0, posm, velr, sig, drho, acc, dsig)
+    assert np.array_equal(po0, posm.astype(np.float64)) and np.array_equal(vo0, velr.astype(np.float64))
+
+
+def test_step_composite_consistency():
+    w = W.t1b(8, 1106)
+    r = orc.step(w.posm, w.velr, w.sig, w.owner, w.origin, w.dims, w.h, w.K, w.G, w.n_owners, w.dt)
+    assert np.array_equal(np.sort(r.perm), np.arange(w.n))
+    assert np.all(np.diff(r.sorted_hash.astype(np.int64)) >= 0)
+    same = np.diff(r.sorted_hash.astype(np.int64)) == 0
+    assert np.all(np.diff(r.perm.astype(np.int64))[same] > 0)       # ids increase inside a bucket
+    # state comes back in id order, mass and owner untouched
+    assert np.array_equal(r.posm[:, 3], w.posm[:, 3].astype(np.float64))
+    acc_id = np.empty((w.n, 3)); acc_id[r.perm] = r.rates.acc
+    assert np.allclose(r.velr[:, :3], w.velr[:, :3].astype(np.float64) + w.dt * acc_id, atol=1e-15)
+
+
+def test_expected_boundary_fractions():
+    """cfg0 ~46.8 %; random labels 100 %; cfg1-like slabs a minority."""
+    w = W.config(0)
+    r, *_ = sorted_view(w)
+    assert abs(r.boundary_ids.size / w.n - 0.468) < 0.02
+    w = W.config(4, side=24)
+    r, *_ = sorted_view(w)
+    assert r.boundary_ids.size == w.n
+    w = W.config(2, side=32)
+    r, *_ = sorted_view(w)
+    assert r.boundary_ids.size == w.n
