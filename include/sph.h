@@ -1,0 +1,174 @@
+/*
+ * sph.h -- C-ABI boundary of the B200-native SPH hot path (libsph_b200.so).
+ *
+ * One iteration of the particle-decomposition SPH scheme of Unfer, Colle & Limido
+ * (arxiv 2310.03596; cited below as PAPER.md:<line> = /root/reference/PAPER.md), restricted to
+ * one GPU: owner labels stand in for the paper's GPUs, the "MGPU boundary
+ * particle" set is the product of stage 3, the multi-GPU broadcasts (steps b, d)
+ * are out of scope.  Readings of everything the paper leaves open (S1..S28) are in DESIGN.md
+ * section 3.
+ *
+ * Conventions
+ *  - "dev"  = CUDA device pointer, owned by the CALLER (e.g. a torch tensor); the library never
+ *    allocates, frees or retains it beyond the call's enqueued work.
+ *    "host" = ordinary host pointer (only sph_params, sph_state structs themselves, and the
+ *    buffers of sph_step_host).
+ *  - sph_ctx owns only scratch (radix-sort ping-pong buffers, histograms, tile status words,
+ *    per-bucket owner masks, scan space, the sorted copy of the state used by sph_step).  It is
+ *    sized for max_n particles and the grid of the sph_params given at creation.
+ *  - Every entry point except sph_create / sph_destroy / sph_step_host only ENQUEUES work on the
+ *    ctx's stream and returns; outputs are valid once the caller synchronises that stream.
+ *    No allocation and no host synchronisation happens on the hot path.  One ctx per host thread.
+ *  - Return value: 0 = SPH_OK, negative = error (below).  No exception crosses this boundary.
+ *  - Per-particle arrays: posm [n][4] = x, y, z, m;  velr [n][4] = vx, vy, vz, rho;
+ *    sig[c] [n], c = xx, yy, zz, xy, xz, yz (SoA);  owner [n] in [0, n_owners).
+ *    All real data fp32, all hashes / indices uint32.  posm / velr / acc must be 16-byte aligned,
+ *    everything else 4-byte aligned.
+ *  - "sorted position k": index in the (hash, id) order produced by sph_sort; perm[k] is the
+ *    persistent particle id (= index in the caller's id-ordered arrays) of the k-th particle.
+ */
+#ifndef SPH_B200_H
+#define SPH_B200_H
+
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+#define SPH_OK        0
+#define SPH_EINVAL   -1   /* null pointer, n < 0, n > max_n, bad params                         */
+#define SPH_ECUDA    -2   /* a CUDA runtime call or launch failed (see sph_last_cuda_error)     */
+#define SPH_ENOMEM   -3   /* scratch allocation failed                                           */
+
+#define SPH_GARBAGE_HASH 0xFFFFFFFFu  /* PAPER.md:17 "some garbage collector hash" (reading S8) */
+#define SPH_MAX_OWNERS   32           /* paper's envelope is <= 16 GPUs           */
+
+/* sph_params.flags */
+#define SPH_FLAG_INTERACT_DIRECT 1u   /* force the simple global-memory interaction kernel      */
+
+typedef struct sph_ctx sph_ctx;      /* opaque */
+
+typedef struct {
+    float    origin[3];  /* lower corner of the bucket grid (reading S3)                        */
+    int32_t  dims[3];    /* nx, ny, nz buckets; nx*ny*nz < 2^32 - 1                              */
+    float    h;          /* uniform smoothing length; bucket edge = support = 2h   */
+    float    K, G;       /* bulk / shear modulus of the linear-elastic law (BASELINE.json cfgs)  */
+    int32_t  n_owners;   /* 1 .. SPH_MAX_OWNERS                                                  */
+    uint32_t flags;      /* SPH_FLAG_* or 0                                                      */
+} sph_params;
+
+typedef struct {          /* SoA particle state; every pointer dev, length n                     */
+    float   *posm;        /* [n][4] x, y, z, m                                                   */
+    float   *velr;        /* [n][4] vx, vy, vz, rho                                              */
+    float   *sig[6];      /* xx, yy, zz, xy, xz, yz                                              */
+    int32_t *owner;       /* [n]                                                                 */
+} sph_state;
+
+/* Create a context: validates params, allocates scratch for max_n particles on the current
+ * device.  cuda_stream is a cudaStream_t (borrowed; NULL = legacy default stream).
+ * Errors: SPH_EINVAL (null, max_n < 0 or >= 2^30, dims <= 0 or product >= 2^32-1, h <= 0 or not
+ * finite, n_owners outside 1..32), SPH_ENOMEM, SPH_ECUDA. */
+int sph_create(sph_ctx **ctx, const sph_params *params, int64_t max_n, void *cuda_stream);
+int sph_destroy(sph_ctx *ctx);
+
+/* Stage 1 -- bucket hash ("Each particle is given a hash number corresponding to the
+ * bucket in which it is located"; step a).  For each axis a, in fp32 and in this
+ * order (reading S2): t = x_a - origin_a; u = t * inv (inv = 1.0f / (2.0f * h), rounded once);
+ * f = floorf(u) clamped to [0, dims_a - 1] (out-of-grid particles are clamped, never an error);
+ * hash = cx + nx * (cy + ny * cz) (reading S1).  Non-finite positions give an unspecified hash.
+ * posm: dev [n][4] in id order.  hash: dev [n] out. */
+int sph_hash(sph_ctx *ctx, int64_t n, const float *posm, uint32_t *hash);
+
+/* Stage 2a -- stable LSD radix sort (hand-written onesweep) on the key (hash, id)
+ * ("sorted with respect to this hash number by the radix sort algorithm"; reading
+ * S5).  hash: dev [n] in id order (index = particle id), every value < nx*ny*nz.
+ * sorted_hash, perm: dev [n] out; perm[k] = id of the k-th particle, sorted_hash[k] =
+ * hash[perm[k]].  Only the ceil(log2(nx*ny*nz)) live key bits are sorted. */
+int sph_sort(sph_ctx *ctx, int64_t n, const uint32_t *hash, uint32_t *sorted_hash, uint32_t *perm);
+
+/* Stage 2b -- gather the state into sorted order: out.X[k] = in.X[perm[k]] for every field
+ * ("The particles are then sorted").  in and out must not alias. */
+int sph_reorder(sph_ctx *ctx, int64_t n, const uint32_t *perm, const sph_state *in,
+                const sph_state *out);
+
+/* Stage 2c -- cell start/end tables (BASELINE.json north_star; reading S7):
+ * cell_start[c] = #{k : sorted_hash[k] < c}, cell_end[c] = #{k : sorted_hash[k] <= c};
+ * both dev [nx*ny*nz] out.  Empty bucket => start == end. */
+int sph_cell_ranges(sph_ctx *ctx, int64_t n, const uint32_t *sorted_hash, uint32_t *cell_start,
+                    uint32_t *cell_end);
+
+/* Stage 3 -- communication hash and MGPU boundary particles (step c PAPER.md:22).
+ * comm_hash[k] = sorted_hash[k] if a particle with a different owner lies in the 27-bucket
+ * stencil of k's bucket (out-of-grid buckets skipped, reading S9; bucket-level test, S10), else
+ * SPH_GARBAGE_HASH.  boundary_ids = ids (perm values) of the particles with comm_hash !=
+ * garbage in ascending (comm_hash, id) order, i.e. the head of the paper's sort on that key
+ * (I6: identical to a stable compaction of the sorted array); *boundary_count = M;
+ * owner_counts[g] = how many of them carry owner g.
+ * In: sorted_hash, sorted_owner, perm dev [n]; cell_start, cell_end dev [cells].
+ * Out: comm_hash dev [n]; boundary_ids dev, capacity n; boundary_count dev scalar;
+ * owner_counts dev [n_owners]. */
+int sph_comm_hash(sph_ctx *ctx, int64_t n, const uint32_t *sorted_hash, const int32_t *sorted_owner,
+                  const uint32_t *perm, const uint32_t *cell_start, const uint32_t *cell_end,
+                  uint32_t *comm_hash, uint32_t *boundary_ids, uint32_t *boundary_count,
+                  uint32_t *owner_counts);
+
+/* Stage 4a -- SPH interaction loops over the 27-bucket stencil (steps e/f
+ * PAPER.md:24-25, "several interaction loops" PAPER.md:28; equations: DESIGN.md O6-O8).
+ * Neighbours of i: every j != i in the stencil of i's bucket with r_ij^2 < (2h)^2.
+ *   drho_i = sum_j m_j (v_i - v_j) . gradW_ij            (density rate)
+ *   L_i    = sum_j (m_j / rho_j) (v_j - v_i) (x) gradW_ij (velocity gradient)
+ *   acc_i  = sum_j m_j (sigma_i / rho_i^2 + sigma_j / rho_j^2) . gradW_ij
+ *   dsig_i = K tr(D) I + 2G dev(D) + Om sigma - sigma Om,  D, Om = sym / skew part of L
+ * with the Wendland C2 kernel, gradW_ij = F(r) x_ij.  All rates use the state at the start of
+ * the step.  `sorted` is the state in sorted order (sorted_hash gives each particle's bucket).
+ * Out (dev, indexed by sorted position): drho [n], acc [n][4] (w = 0), dsig[c] [n].
+ * pair_count: dev scalar or NULL; receives the number of ordered accepted pairs (reading S25). */
+int sph_interact(sph_ctx *ctx, int64_t n, const sph_state *sorted, const uint32_t *sorted_hash,
+                 const uint32_t *cell_start, const uint32_t *cell_end, float *drho, float *acc,
+                 float *const dsig[6], unsigned long long *pair_count);
+
+/* Stage 4b -- explicit integration, symplectic Euler (step g; reading S18):
+ * rho += dt drho; v += dt acc; sigma += dt dsig; x += dt v(new).  m and owner are copied.
+ * Elementwise: in, rates and out use the same index order; out may alias in. */
+int sph_integrate(sph_ctx *ctx, int64_t n, float dt, const sph_state *in, const float *drho,
+                  const float *acc, const float *const dsig[6], const sph_state *out);
+
+/* The whole iteration on one stream, no host synchronisation (PAPER.md:19-26 with steps b, d
+ * removed): hash -> sort -> reorder -> cell ranges -> comm hash + compaction -> interact ->
+ * integrate.  `state` is in ID ORDER on entry and on exit (so the (hash, id) tie-break stays
+ * exact when every step re-sorts, reading S5).  Every output pointer below is optional (NULL =
+ * keep it in ctx scratch); when given it receives exactly what the stage call of the same name
+ * would produce (rates indexed by sorted position). */
+int sph_step(sph_ctx *ctx, int64_t n, float dt, const sph_state *state,
+             uint32_t *hash, uint32_t *sorted_hash, uint32_t *perm,
+             uint32_t *cell_start, uint32_t *cell_end, uint32_t *comm_hash,
+             uint32_t *boundary_ids, uint32_t *boundary_count, uint32_t *owner_counts,
+             float *drho, float *acc, float *const dsig[6], unsigned long long *pair_count);
+
+/* End-to-end variant with HOST buffers (pinned memory recommended): uploads the id-ordered state,
+ * runs `steps` iterations, downloads the state, the boundary list of the last step and the
+ * counters, and synchronises the stream before returning.  Device staging lives in the ctx
+ * (allocated on first use).  host_state pointers are host; boundary_ids host capacity n (may be
+ * NULL); boundary_count / pair_count host scalars (may be NULL; pair_count accumulates over the
+ * steps). */
+int sph_step_host(sph_ctx *ctx, int64_t n, float dt, int32_t steps, const sph_state *host_state,
+                  uint32_t *boundary_ids, uint32_t *boundary_count, unsigned long long *pair_count);
+
+/* Per-stage device time of the most recent sph_step, measured with CUDA events recorded on the
+ * ctx's stream (enabled by sph_enable_timing(ctx, 1); adds no host sync to sph_step itself --
+ * this call synchronises).  ms[0..7] = hash, sort, reorder, cell_ranges, comm_hash, interact,
+ * integrate, total. */
+int sph_enable_timing(sph_ctx *ctx, int32_t on);
+int sph_get_timing(sph_ctx *ctx, float ms[8]);
+
+/* How many kernels the library has launched through this ctx since creation. */
+int64_t sph_launch_count(const sph_ctx *ctx);
+
+const char *sph_strerror(int code);
+const char *sph_last_cuda_error(const sph_ctx *ctx);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* SPH_B200_H */

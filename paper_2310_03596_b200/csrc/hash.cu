@@ -1,0 +1,52 @@
+// Stage 1: bucket hash (step a PAPER.md:19; readings S1-S3).
+// Pure streaming kernel: 16 B read + 4 B written per particle, HBM-bound.
+#include "sph_internal.cuh"
+
+namespace sphb {
+
+__device__ __forceinline__ uint32_t bucket_coord(float x, float o, float inv, int n)
+{
+    // fp32 sequence pinned by reading S2: sub, mul, floor, clamp (no contraction possible)
+    float t = __fsub_rn(x, o);
+    float u = __fmul_rn(t, inv);
+    float f = floorf(u);
+    float top = (float)(n - 1);
+    f = f < 0.0f ? 0.0f : f;
+    f = f > top ? top : f;
+    return (uint32_t)(int)f;
+}
+
+__global__ void __launch_bounds__(256) hash_kernel(int64_t n, const float4 *__restrict__ posm,
+                                                   uint32_t *__restrict__ hash, Grid g)
+{
+    // two particles per thread, both loads issued before use
+    int64_t i0 = ((int64_t)blockIdx.x * blockDim.x) * 2 + threadIdx.x;
+    int64_t i1 = i0 + blockDim.x;
+    float4 p0, p1;
+    if (i0 < n) p0 = __ldcs(posm + i0);
+    if (i1 < n) p1 = __ldcs(posm + i1);
+    if (i0 < n) {
+        uint32_t cx = bucket_coord(p0.x, g.ox, g.inv_edge, g.nx);
+        uint32_t cy = bucket_coord(p0.y, g.oy, g.inv_edge, g.ny);
+        uint32_t cz = bucket_coord(p0.z, g.oz, g.inv_edge, g.nz);
+        hash[i0] = cx + (uint32_t)g.nx * (cy + (uint32_t)g.ny * cz);
+    }
+    if (i1 < n) {
+        uint32_t cx = bucket_coord(p1.x, g.ox, g.inv_edge, g.nx);
+        uint32_t cy = bucket_coord(p1.y, g.oy, g.inv_edge, g.ny);
+        uint32_t cz = bucket_coord(p1.z, g.oz, g.inv_edge, g.nz);
+        hash[i1] = cx + (uint32_t)g.nx * (cy + (uint32_t)g.ny * cz);
+    }
+}
+
+int launch_hash(sph_ctx *c, int64_t n, const float *posm, uint32_t *hash)
+{
+    if (n == 0) return SPH_OK;
+    int blocks = div_up(n, 512);
+    hash_kernel<<<blocks, 256, 0, c->stream>>>(n, reinterpret_cast<const float4 *>(posm), hash,
+                                               c->grid);
+    SPH_CHECK_LAUNCH(c);
+    return SPH_OK;
+}
+
+}  // namespace sphb

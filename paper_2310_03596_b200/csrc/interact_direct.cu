@@ -1,0 +1,78 @@
+// Stage 4a, reference-shaped kernel: one thread per particle walking the 27-bucket stencil
+// straight out of global memory ("restricted to its bucket and to the surrounding
+// buckets"; steps e/f PAPER.md:24-25; equations DESIGN.md O6-O8).
+//
+// This is the simple first CUDA path and the fallback for tiles that do not fit the shared-
+// memory kernel in interact_tiled.cu.  x-fastest hashing makes the three buckets (cx-1, cx,
+// cx+1) of a stencil row contiguous, so the 27 buckets are 9 contiguous runs.
+#include "sph_internal.cuh"
+#include "interact_math.cuh"
+
+namespace sphb {
+
+__global__ void __launch_bounds__(128)
+interact_direct_kernel(int64_t n, InteractIn in, const uint32_t *__restrict__ sorted_hash,
+                       const uint32_t *__restrict__ cs, const uint32_t *__restrict__ ce, Grid g,
+                       Consts k, InteractOut out, unsigned long long *pair_count)
+{
+    const int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    unsigned long long my_pairs = 0;
+    if (i < n) {
+        const uint32_t h = sorted_hash[i];
+        const int cx = h % g.nx, cy = (h / g.nx) % g.ny, cz = h / (g.nx * g.ny);
+        const float4 pi = in.posm[i];
+        const float4 vi = in.velr[i];
+        PairAccum A;
+        A.clear();
+        const int x0 = max(cx - 1, 0), x1 = min(cx + 1, g.nx - 1);
+        for (int dz = -1; dz <= 1; ++dz) {
+            const int z = cz + dz;
+            if (z < 0 || z >= g.nz) continue;
+            for (int dy = -1; dy <= 1; ++dy) {
+                const int y = cy + dy;
+                if (y < 0 || y >= g.ny) continue;
+                const uint32_t row = (uint32_t)g.nx * ((uint32_t)y + (uint32_t)g.ny * (uint32_t)z);
+                const uint32_t jb = cs[row + x0], je = ce[row + x1];
+                for (uint32_t j = jb; j < je; ++j) {
+                    const float4 pj = in.posm[j];
+                    const float dx = pi.x - pj.x, dy_ = pi.y - pj.y, dz_ = pi.z - pj.z;
+                    const float r2 = dx * dx + dy_ * dy_ + dz_ * dz_;
+                    if (r2 < k.support2 && j != (uint32_t)i) {
+                        const float4 vj = in.velr[j];
+                        const float inv_rho = 1.0f / vj.w;
+                        const float Vj = pj.w * inv_rho;
+                        const float ir2 = inv_rho * inv_rho;
+                        float Sj[6];
+#pragma unroll
+                        for (int c = 0; c < 6; ++c) Sj[c] = in.sig[c][j] * ir2;
+                        A.add(dx, dy_, dz_, r2, pj.w, Vj, vj.x - vi.x, vj.y - vi.y, vj.z - vi.z, Sj,
+                              k.half_inv_h);
+                        ++my_pairs;
+                    }
+                }
+            }
+        }
+        float si[6];
+#pragma unroll
+        for (int c = 0; c < 6; ++c) si[c] = in.sig[c][i];
+        finish_particle(A, si, vi.w, k, out, i);
+    }
+    if (pair_count) {
+        // warp, then one atomic per warp
+#pragma unroll
+        for (int o = 16; o > 0; o >>= 1) my_pairs += __shfl_xor_sync(0xffffffffu, my_pairs, o);
+        if ((threadIdx.x & 31) == 0 && my_pairs) atomicAdd(pair_count, my_pairs);
+    }
+}
+
+int launch_interact_direct(sph_ctx *c, int64_t n, const InteractIn &in, const uint32_t *sorted_hash,
+                           const uint32_t *cs, const uint32_t *ce, const InteractOut &out,
+                           unsigned long long *pair_count)
+{
+    interact_direct_kernel<<<div_up(n, 128), 128, 0, c->stream>>>(n, in, sorted_hash, cs, ce, c->grid,
+                                                                  c->consts, out, pair_count);
+    SPH_CHECK_LAUNCH(c);
+    return SPH_OK;
+}
+
+}  // namespace sphb

@@ -1,0 +1,111 @@
+// Pair arithmetic shared by the two interaction kernels (O6-O8, fp32).
+//
+// Wendland C2, support 2h: grad_i W_ij = F(r) x_ij, F(r) = cF (1 - r/2h)^3, cF = -5 alpha / h^2.
+// The constant cF is applied once per particle; per pair only t^3 is formed.
+//   drho_i = sum_j m_j (v_i - v_j).gradW        = -cF sum (m_j t^3 x_ij) . dv,  dv = v_j - v_i
+//   L_ab   = sum_j V_j dv_a gradW_b             =  cF sum dv_a (V_j t^3 x_ij)_b
+//   acc_i  = sum_j m_j (S_i + S_j) gradW        =  cF [ S_i g + sum S_j (m_j t^3 x_ij) ],
+//            g = sum m_j t^3 x_ij,  S = sigma / rho^2,  V = m / rho.
+#pragma once
+#include "sph_internal.cuh"
+
+namespace sphb {
+
+struct InteractIn {
+    const float4 *posm, *velr;
+    const float *sig[6];
+};
+struct InteractOut {
+    float *drho;
+    float4 *acc;
+    float *dsig[6];
+};
+
+struct PairAccum {
+    float dr;          // sum dv . mx
+    float L[9];        // sum dv_a * wx_b
+    float g[3];        // sum mx
+    float a[3];        // sum S_j mx
+    __device__ __forceinline__ void clear()
+    {
+        dr = 0.f;
+#pragma unroll
+        for (int i = 0; i < 9; ++i) L[i] = 0.f;
+#pragma unroll
+        for (int i = 0; i < 3; ++i) { g[i] = 0.f; a[i] = 0.f; }
+    }
+    // S = (xx, yy, zz, xy, xz, yz) of sigma_j / rho_j^2
+    __device__ __forceinline__ void add(float dx, float dy, float dz, float r2, float mj, float Vj,
+                                        float dvx, float dvy, float dvz, const float (&S)[6],
+                                        float half_inv_h)
+    {
+        const float r2c = fmaxf(r2, 1e-30f);          // coincident particles: gradW = 0 (S15)
+        const float r = r2c * rsqrtf(r2c);
+        const float t = fmaf(r, -half_inv_h, 1.0f);
+        const float F = t * t * t;
+        const float wm = mj * F, wV = Vj * F;
+        const float mx = wm * dx, my = wm * dy, mz = wm * dz;
+        const float wx = wV * dx, wy = wV * dy, wz = wV * dz;
+        dr = fmaf(dvx, mx, dr); dr = fmaf(dvy, my, dr); dr = fmaf(dvz, mz, dr);
+        L[0] = fmaf(dvx, wx, L[0]); L[1] = fmaf(dvx, wy, L[1]); L[2] = fmaf(dvx, wz, L[2]);
+        L[3] = fmaf(dvy, wx, L[3]); L[4] = fmaf(dvy, wy, L[4]); L[5] = fmaf(dvy, wz, L[5]);
+        L[6] = fmaf(dvz, wx, L[6]); L[7] = fmaf(dvz, wy, L[7]); L[8] = fmaf(dvz, wz, L[8]);
+        g[0] += mx; g[1] += my; g[2] += mz;
+        a[0] = fmaf(S[0], mx, a[0]); a[0] = fmaf(S[3], my, a[0]); a[0] = fmaf(S[4], mz, a[0]);
+        a[1] = fmaf(S[3], mx, a[1]); a[1] = fmaf(S[1], my, a[1]); a[1] = fmaf(S[5], mz, a[1]);
+        a[2] = fmaf(S[4], mx, a[2]); a[2] = fmaf(S[5], my, a[2]); a[2] = fmaf(S[2], mz, a[2]);
+    }
+};
+
+// Per-particle epilogue: scale by cF, add the S_i term, form the stress rate (O8) and store.
+__device__ __forceinline__ void finish_particle(const PairAccum &A, const float (&sig_i)[6],
+                                                float rho_i, const Consts &k, const InteractOut &out,
+                                                int64_t i)
+{
+    const float cF = k.cF;
+    const float ir = 1.0f / rho_i;
+    const float ir2 = ir * ir;
+    const float Sxx = sig_i[0] * ir2, Syy = sig_i[1] * ir2, Szz = sig_i[2] * ir2;
+    const float Sxy = sig_i[3] * ir2, Sxz = sig_i[4] * ir2, Syz = sig_i[5] * ir2;
+    float4 acc;
+    acc.x = cF * (A.a[0] + Sxx * A.g[0] + Sxy * A.g[1] + Sxz * A.g[2]);
+    acc.y = cF * (A.a[1] + Sxy * A.g[0] + Syy * A.g[1] + Syz * A.g[2]);
+    acc.z = cF * (A.a[2] + Sxz * A.g[0] + Syz * A.g[1] + Szz * A.g[2]);
+    acc.w = 0.f;
+    out.drho[i] = -cF * A.dr;
+    out.acc[i] = acc;
+    float L[9];
+#pragma unroll
+    for (int q = 0; q < 9; ++q) L[q] = cF * A.L[q];
+    // D = sym(L), Om = skew(L);  dsig = K trD I + 2G (D - trD/3 I) + Om sig - sig Om
+    const float Dxx = L[0], Dyy = L[4], Dzz = L[8];
+    const float Dxy = 0.5f * (L[1] + L[3]), Dxz = 0.5f * (L[2] + L[6]), Dyz = 0.5f * (L[5] + L[7]);
+    const float Oxy = 0.5f * (L[1] - L[3]), Oxz = 0.5f * (L[2] - L[6]), Oyz = 0.5f * (L[5] - L[7]);
+    const float trD = Dxx + Dyy + Dzz;
+    const float vol = (k.K - (2.0f / 3.0f) * k.G) * trD;
+    const float G2 = 2.0f * k.G;
+    const float sxx = sig_i[0], syy = sig_i[1], szz = sig_i[2], sxy = sig_i[3], sxz = sig_i[4],
+                syz = sig_i[5];
+    // (Om s - s Om) for skew Om = [[0,Oxy,Oxz],[-Oxy,0,Oyz],[-Oxz,-Oyz,0]] and symmetric s
+    const float Jxx = 2.0f * (Oxy * sxy + Oxz * sxz);
+    const float Jyy = 2.0f * (-Oxy * sxy + Oyz * syz);
+    const float Jzz = -2.0f * (Oxz * sxz + Oyz * syz);
+    const float Jxy = Oxy * (syy - sxx) + Oxz * syz + Oyz * sxz;
+    const float Jxz = Oxz * (szz - sxx) + Oxy * syz - Oyz * sxy;
+    const float Jyz = Oyz * (szz - syy) - Oxy * sxz - Oxz * sxy;
+    out.dsig[0][i] = vol + G2 * Dxx + Jxx;
+    out.dsig[1][i] = vol + G2 * Dyy + Jyy;
+    out.dsig[2][i] = vol + G2 * Dzz + Jzz;
+    out.dsig[3][i] = G2 * Dxy + Jxy;
+    out.dsig[4][i] = G2 * Dxz + Jxz;
+    out.dsig[5][i] = G2 * Dyz + Jyz;
+}
+
+int launch_interact_direct(sph_ctx *c, int64_t n, const InteractIn &in, const uint32_t *sorted_hash,
+                           const uint32_t *cs, const uint32_t *ce, const InteractOut &out,
+                           unsigned long long *pair_count);
+int launch_interact_tiled(sph_ctx *c, int64_t n, const InteractIn &in, const uint32_t *sorted_hash,
+                          const uint32_t *cs, const uint32_t *ce, const InteractOut &out,
+                          unsigned long long *pair_count);
+
+}  // namespace sphb

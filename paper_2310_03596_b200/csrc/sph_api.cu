@@ -1,0 +1,375 @@
+// C-ABI entry points of libsph_b200.so (include/sph.h): argument checks, scratch management and
+// the per-iteration sequence of PAPER.md:19-26 on one stream.
+#include <math.h>
+#include <new>
+#include <string.h>
+
+#include "sph_internal.cuh"
+
+using namespace sphb;
+
+namespace {
+
+size_t align_up(size_t v, size_t a) { return (v + a - 1) / a * a; }
+
+struct Carver {
+    char *base;
+    size_t off;
+    template <typename T> T *take(size_t count)
+    {
+        off = align_up(off, 256);
+        T *p = base ? reinterpret_cast<T *>(base + off) : nullptr;
+        off += count * sizeof(T);
+        return p;
+    }
+};
+
+int ceil_log2_u64(uint64_t v)
+{
+    int b = 0;
+    while ((1ull << b) < v) ++b;
+    return b;
+}
+
+void carve(sph_ctx *c, char *base, size_t *total)
+{
+    Carver k{base, 0};
+    const size_t n = (size_t)(c->max_n > 0 ? c->max_n : 1);
+    const size_t cells = c->grid.n_cells;
+    const size_t tiles = (n + kSortTile - 1) / kSortTile;
+    const size_t scan_n = cells > n ? cells : n;
+    const size_t scan_tiles = (scan_n + kScanTile - 1) / kScanTile;
+    c->alt_keys = k.take<uint32_t>(n);
+    c->alt_vals = k.take<uint32_t>(n);
+    c->hist = k.take<uint32_t>(kMaxPasses * kRadix);
+    c->tile_status = k.take<uint32_t>((size_t)(c->n_passes > 0 ? c->n_passes : 1) * tiles * kRadix);
+    c->tile_counter = k.take<uint32_t>(kMaxPasses + 2);
+    c->cell_mask = k.take<uint32_t>(cells);
+    c->cell_flag_count = k.take<uint32_t>(cells);
+    c->cell_offset = k.take<uint32_t>(cells);
+    c->scan_status = k.take<uint32_t>(scan_tiles);
+    c->s_hash = k.take<uint32_t>(n);
+    c->s_sorted_hash = k.take<uint32_t>(n);
+    c->s_perm = k.take<uint32_t>(n);
+    c->s_cell_start = k.take<uint32_t>(cells);
+    c->s_cell_end = k.take<uint32_t>(cells);
+    c->s_comm_hash = k.take<uint32_t>(n);
+    c->s_boundary_ids = k.take<uint32_t>(n);
+    c->s_boundary_count = k.take<uint32_t>(4);
+    c->s_owner_counts = k.take<uint32_t>(SPH_MAX_OWNERS);
+    c->s_drho = k.take<float>(n);
+    c->s_acc = k.take<float>(4 * n);
+    for (int i = 0; i < 6; ++i) c->s_dsig[i] = k.take<float>(n);
+    c->s_pair_count = k.take<unsigned long long>(2);
+    c->sorted.posm = k.take<float>(4 * n);
+    c->sorted.velr = k.take<float>(4 * n);
+    for (int i = 0; i < 6; ++i) c->sorted.sig[i] = k.take<float>(n);
+    c->sorted.owner = k.take<int32_t>(n);
+    *total = align_up(k.off, 256);
+}
+
+bool state_ok(const sph_state *s)
+{
+    if (!s || !s->posm || !s->velr || !s->owner) return false;
+    for (int i = 0; i < 6; ++i)
+        if (!s->sig[i]) return false;
+    return true;
+}
+
+bool n_ok(const sph_ctx *c, int64_t n) { return c && n >= 0 && n <= c->max_n; }
+
+struct StageTimer {
+    sph_ctx *c;
+    int idx = 0;
+    explicit StageTimer(sph_ctx *ctx) : c(ctx) { mark(); }
+    void mark()
+    {
+        if (c->timing.on) cudaEventRecord(c->timing.ev[idx], c->stream);
+        ++idx;
+    }
+};
+
+}  // namespace
+
+extern "C" {
+
+static int step_impl(sph_ctx *c, int64_t n, float dt, const sph_state *state, uint32_t *hash,
+                     uint32_t *sorted_hash, uint32_t *perm, uint32_t *cell_start, uint32_t *cell_end,
+                     uint32_t *comm_hash, uint32_t *boundary_ids, uint32_t *boundary_count,
+                     uint32_t *owner_counts, float *drho, float *acc, float *const dsig[6],
+                     unsigned long long *pair_count, bool zero_pairs);
+
+int sph_create(sph_ctx **out, const sph_params *p, int64_t max_n, void *cuda_stream)
+{
+    if (!out || !p) return SPH_EINVAL;
+    *out = nullptr;
+    if (max_n < 0 || max_n >= (1ll << 30)) return SPH_EINVAL;
+    if (!(p->h > 0.0f) || !isfinite(p->h)) return SPH_EINVAL;
+    if (p->n_owners < 1 || p->n_owners > SPH_MAX_OWNERS) return SPH_EINVAL;
+    uint64_t cells = 1;
+    for (int a = 0; a < 3; ++a) {
+        if (p->dims[a] <= 0) return SPH_EINVAL;
+        cells *= (uint64_t)p->dims[a];
+        if (cells >= 0xFFFFFFFFull) return SPH_EINVAL;
+    }
+    if (!isfinite(p->origin[0]) || !isfinite(p->origin[1]) || !isfinite(p->origin[2])) return SPH_EINVAL;
+
+    sph_ctx *c = new (std::nothrow) sph_ctx();
+    if (!c) return SPH_ENOMEM;
+    c->params = *p;
+    c->max_n = max_n;
+    c->stream = reinterpret_cast<cudaStream_t>(cuda_stream);
+    c->launches = 0;
+    c->last_err = cudaSuccess;
+    c->staging_ready = false;
+    memset(&c->staging, 0, sizeof(c->staging));
+
+    // grid constants: inv_edge rounded once in fp32 (reading S2)
+    const float edge = 2.0f * p->h;
+    c->grid.ox = p->origin[0]; c->grid.oy = p->origin[1]; c->grid.oz = p->origin[2];
+    c->grid.inv_edge = 1.0f / edge;
+    c->grid.nx = p->dims[0]; c->grid.ny = p->dims[1]; c->grid.nz = p->dims[2];
+    c->grid.n_cells = (uint32_t)cells;
+    // kernel constants (computed in double, rounded once)
+    const double h = (double)p->h;
+    const double alpha = 21.0 / (16.0 * 3.14159265358979323846 * h * h * h);
+    c->consts.support2 = edge * edge;
+    c->consts.half_inv_h = (float)(0.5 / h);
+    c->consts.cF = (float)(-5.0 * alpha / (h * h));
+    c->consts.K = p->K;
+    c->consts.G = p->G;
+    c->key_bits = ceil_log2_u64(cells);
+    c->n_passes = (c->key_bits + kRadixBits - 1) / kRadixBits;
+
+    cudaError_t e = cudaGetDevice(&c->device);
+    if (e == cudaSuccess) e = cudaDeviceGetAttribute(&c->num_sms, cudaDevAttrMultiProcessorCount, c->device);
+    if (e != cudaSuccess) { delete c; return SPH_ECUDA; }
+
+    size_t total = 0;
+    carve(c, nullptr, &total);
+    c->arena_bytes = total;
+    e = cudaMalloc(&c->arena, total);
+    if (e != cudaSuccess) { cudaGetLastError(); delete c; return SPH_ENOMEM; }
+    carve(c, static_cast<char *>(c->arena), &total);
+    for (int i = 0; i < 9; ++i) {
+        if (cudaEventCreate(&c->timing.ev[i]) != cudaSuccess) { cudaFree(c->arena); delete c; return SPH_ECUDA; }
+    }
+    *out = c;
+    return SPH_OK;
+}
+
+int sph_destroy(sph_ctx *c)
+{
+    if (!c) return SPH_EINVAL;
+    cudaStreamSynchronize(c->stream);
+    for (int i = 0; i < 9; ++i) cudaEventDestroy(c->timing.ev[i]);
+    if (c->staging_ready) {
+        cudaFree(c->staging.posm);
+    }
+    cudaFree(c->arena);
+    delete c;
+    return SPH_OK;
+}
+
+int sph_hash(sph_ctx *c, int64_t n, const float *posm, uint32_t *hash)
+{
+    if (!n_ok(c, n) || !posm || !hash) return SPH_EINVAL;
+    return launch_hash(c, n, posm, hash);
+}
+
+int sph_sort(sph_ctx *c, int64_t n, const uint32_t *hash, uint32_t *sorted_hash, uint32_t *perm)
+{
+    if (!n_ok(c, n) || !hash || !sorted_hash || !perm) return SPH_EINVAL;
+    return launch_sort(c, n, hash, sorted_hash, perm);
+}
+
+int sph_reorder(sph_ctx *c, int64_t n, const uint32_t *perm, const sph_state *in, const sph_state *out)
+{
+    if (!n_ok(c, n) || !perm || !state_ok(in) || !state_ok(out)) return SPH_EINVAL;
+    return launch_reorder(c, n, perm, in, out);
+}
+
+int sph_cell_ranges(sph_ctx *c, int64_t n, const uint32_t *sorted_hash, uint32_t *cs, uint32_t *ce)
+{
+    if (!n_ok(c, n) || !sorted_hash || !cs || !ce) return SPH_EINVAL;
+    return launch_cell_ranges(c, n, sorted_hash, cs, ce);
+}
+
+int sph_comm_hash(sph_ctx *c, int64_t n, const uint32_t *sorted_hash, const int32_t *sorted_owner,
+                  const uint32_t *perm, const uint32_t *cs, const uint32_t *ce, uint32_t *comm_hash,
+                  uint32_t *boundary_ids, uint32_t *boundary_count, uint32_t *owner_counts)
+{
+    if (!n_ok(c, n) || !sorted_hash || !sorted_owner || !perm || !cs || !ce || !comm_hash ||
+        !boundary_ids || !boundary_count || !owner_counts)
+        return SPH_EINVAL;
+    return launch_comm_hash(c, n, sorted_hash, sorted_owner, perm, cs, ce, comm_hash, boundary_ids,
+                            boundary_count, owner_counts);
+}
+
+int sph_interact(sph_ctx *c, int64_t n, const sph_state *sorted, const uint32_t *sorted_hash,
+                 const uint32_t *cs, const uint32_t *ce, float *drho, float *acc,
+                 float *const dsig[6], unsigned long long *pair_count)
+{
+    if (!n_ok(c, n) || !state_ok(sorted) || !sorted_hash || !cs || !ce || !drho || !acc || !dsig)
+        return SPH_EINVAL;
+    for (int i = 0; i < 6; ++i)
+        if (!dsig[i]) return SPH_EINVAL;
+    if (pair_count)
+        SPH_CUDA_TRY(c, cudaMemsetAsync(pair_count, 0, sizeof(unsigned long long), c->stream));
+    return launch_interact(c, n, sorted, sorted_hash, cs, ce, drho, acc, dsig, pair_count);
+}
+
+int sph_integrate(sph_ctx *c, int64_t n, float dt, const sph_state *in, const float *drho,
+                  const float *acc, const float *const dsig[6], const sph_state *out)
+{
+    if (!n_ok(c, n) || !state_ok(in) || !state_ok(out) || !drho || !acc || !dsig) return SPH_EINVAL;
+    for (int i = 0; i < 6; ++i)
+        if (!dsig[i]) return SPH_EINVAL;
+    return launch_integrate(c, n, dt, in, drho, acc, dsig, out, nullptr);
+}
+
+static int step_impl(sph_ctx *c, int64_t n, float dt, const sph_state *state, uint32_t *hash,
+                     uint32_t *sorted_hash, uint32_t *perm, uint32_t *cell_start, uint32_t *cell_end,
+                     uint32_t *comm_hash, uint32_t *boundary_ids, uint32_t *boundary_count,
+                     uint32_t *owner_counts, float *drho, float *acc, float *const dsig[6],
+                     unsigned long long *pair_count, bool zero_pairs)
+{
+    if (!n_ok(c, n) || !state_ok(state)) return SPH_EINVAL;
+    if (pair_count && zero_pairs)
+        SPH_CUDA_TRY(c, cudaMemsetAsync(pair_count, 0, sizeof(unsigned long long), c->stream));
+    if (!hash) hash = c->s_hash;
+    if (!sorted_hash) sorted_hash = c->s_sorted_hash;
+    if (!perm) perm = c->s_perm;
+    if (!cell_start) cell_start = c->s_cell_start;
+    if (!cell_end) cell_end = c->s_cell_end;
+    if (!comm_hash) comm_hash = c->s_comm_hash;
+    if (!boundary_ids) boundary_ids = c->s_boundary_ids;
+    if (!boundary_count) boundary_count = c->s_boundary_count;
+    if (!owner_counts) owner_counts = c->s_owner_counts;
+    if (!drho) drho = c->s_drho;
+    if (!acc) acc = c->s_acc;
+    float *ds[6];
+    for (int i = 0; i < 6; ++i) ds[i] = (dsig && dsig[i]) ? dsig[i] : c->s_dsig[i];
+
+    int rc;
+    StageTimer t(c);
+    if ((rc = launch_hash(c, n, state->posm, hash)) != SPH_OK) return rc;                  // step a
+    t.mark();
+    if ((rc = launch_sort(c, n, hash, sorted_hash, perm)) != SPH_OK) return rc;
+    t.mark();
+    if ((rc = launch_reorder(c, n, perm, state, &c->sorted)) != SPH_OK) return rc;
+    t.mark();
+    if ((rc = launch_cell_ranges(c, n, sorted_hash, cell_start, cell_end)) != SPH_OK) return rc;
+    t.mark();
+    if ((rc = launch_comm_hash(c, n, sorted_hash, c->sorted.owner, perm, cell_start, cell_end,   // step c
+                               comm_hash, boundary_ids, boundary_count, owner_counts)) != SPH_OK)
+        return rc;
+    t.mark();
+    if ((rc = launch_interact(c, n, &c->sorted, sorted_hash, cell_start, cell_end, drho, acc, ds,  // e, f
+                              pair_count)) != SPH_OK)
+        return rc;
+    t.mark();
+    const float *cds[6] = {ds[0], ds[1], ds[2], ds[3], ds[4], ds[5]};
+    if ((rc = launch_integrate(c, n, dt, &c->sorted, drho, acc, cds, state, perm)) != SPH_OK)    // step g
+        return rc;
+    t.mark();
+    return SPH_OK;
+}
+
+int sph_step(sph_ctx *c, int64_t n, float dt, const sph_state *state, uint32_t *hash,
+             uint32_t *sorted_hash, uint32_t *perm, uint32_t *cell_start, uint32_t *cell_end,
+             uint32_t *comm_hash, uint32_t *boundary_ids, uint32_t *boundary_count,
+             uint32_t *owner_counts, float *drho, float *acc, float *const dsig[6],
+             unsigned long long *pair_count)
+{
+    return step_impl(c, n, dt, state, hash, sorted_hash, perm, cell_start, cell_end, comm_hash,
+                     boundary_ids, boundary_count, owner_counts, drho, acc, dsig, pair_count, true);
+}
+
+int sph_step_host(sph_ctx *c, int64_t n, float dt, int32_t steps, const sph_state *hs,
+                  uint32_t *boundary_ids, uint32_t *boundary_count, unsigned long long *pair_count)
+{
+    if (!n_ok(c, n) || !state_ok(hs) || steps < 0) return SPH_EINVAL;
+    if (!c->staging_ready) {
+        const size_t m = (size_t)(c->max_n > 0 ? c->max_n : 1);
+        char *base = nullptr;
+        // posm 16, velr 16, sig 24, owner 4 bytes per particle, each block 256-aligned
+        const size_t bytes = align_up(16 * m, 256) * 2 + align_up(4 * m, 256) * 7;
+        if (cudaMalloc(&base, bytes) != cudaSuccess) { cudaGetLastError(); return SPH_ENOMEM; }
+        Carver k{base, 0};
+        c->staging.posm = k.take<float>(4 * m);
+        c->staging.velr = k.take<float>(4 * m);
+        for (int i = 0; i < 6; ++i) c->staging.sig[i] = k.take<float>(m);
+        c->staging.owner = k.take<int32_t>(m);
+        c->staging_ready = true;
+    }
+    const sph_state &d = c->staging;
+    cudaStream_t s = c->stream;
+    const size_t nn = (size_t)n;
+    SPH_CUDA_TRY(c, cudaMemcpyAsync(d.posm, hs->posm, 16 * nn, cudaMemcpyHostToDevice, s));
+    SPH_CUDA_TRY(c, cudaMemcpyAsync(d.velr, hs->velr, 16 * nn, cudaMemcpyHostToDevice, s));
+    for (int i = 0; i < 6; ++i)
+        SPH_CUDA_TRY(c, cudaMemcpyAsync(d.sig[i], hs->sig[i], 4 * nn, cudaMemcpyHostToDevice, s));
+    SPH_CUDA_TRY(c, cudaMemcpyAsync(d.owner, hs->owner, 4 * nn, cudaMemcpyHostToDevice, s));
+    SPH_CUDA_TRY(c, cudaMemsetAsync(c->s_pair_count, 0, 2 * sizeof(unsigned long long), s));
+    for (int32_t it = 0; it < steps; ++it) {
+        int rc = step_impl(c, n, dt, &d, nullptr, nullptr, nullptr, nullptr, nullptr, nullptr, nullptr,
+                           nullptr, nullptr, nullptr, nullptr, nullptr, c->s_pair_count, false);
+        if (rc != SPH_OK) return rc;
+    }
+    SPH_CUDA_TRY(c, cudaMemcpyAsync(hs->posm, d.posm, 16 * nn, cudaMemcpyDeviceToHost, s));
+    SPH_CUDA_TRY(c, cudaMemcpyAsync(hs->velr, d.velr, 16 * nn, cudaMemcpyDeviceToHost, s));
+    for (int i = 0; i < 6; ++i)
+        SPH_CUDA_TRY(c, cudaMemcpyAsync(hs->sig[i], d.sig[i], 4 * nn, cudaMemcpyDeviceToHost, s));
+    uint32_t m_host = 0;
+    if (steps > 0 && (boundary_ids || boundary_count)) {
+        SPH_CUDA_TRY(c, cudaMemcpyAsync(&m_host, c->s_boundary_count, sizeof(uint32_t),
+                                        cudaMemcpyDeviceToHost, s));
+        SPH_CUDA_TRY(c, cudaStreamSynchronize(s));
+        if (boundary_ids && m_host)
+            SPH_CUDA_TRY(c, cudaMemcpyAsync(boundary_ids, c->s_boundary_ids, sizeof(uint32_t) * m_host,
+                                            cudaMemcpyDeviceToHost, s));
+    }
+    if (boundary_count) *boundary_count = m_host;
+    if (pair_count)
+        SPH_CUDA_TRY(c, cudaMemcpyAsync(pair_count, c->s_pair_count, sizeof(unsigned long long),
+                                        cudaMemcpyDeviceToHost, s));
+    SPH_CUDA_TRY(c, cudaStreamSynchronize(s));
+    return SPH_OK;
+}
+
+int sph_enable_timing(sph_ctx *c, int32_t on)
+{
+    if (!c) return SPH_EINVAL;
+    c->timing.on = on != 0;
+    return SPH_OK;
+}
+
+int sph_get_timing(sph_ctx *c, float ms[8])
+{
+    if (!c || !ms) return SPH_EINVAL;
+    SPH_CUDA_TRY(c, cudaStreamSynchronize(c->stream));
+    for (int i = 0; i < 7; ++i) SPH_CUDA_TRY(c, cudaEventElapsedTime(&ms[i], c->timing.ev[i], c->timing.ev[i + 1]));
+    SPH_CUDA_TRY(c, cudaEventElapsedTime(&ms[7], c->timing.ev[0], c->timing.ev[7]));
+    return SPH_OK;
+}
+
+int64_t sph_launch_count(const sph_ctx *c) { return c ? c->launches : -1; }
+
+const char *sph_strerror(int code)
+{
+    switch (code) {
+    case SPH_OK: return "ok";
+    case SPH_EINVAL: return "invalid argument";
+    case SPH_ECUDA: return "CUDA error";
+    case SPH_ENOMEM: return "out of device memory";
+    default: return "unknown error";
+    }
+}
+
+const char *sph_last_cuda_error(const sph_ctx *c)
+{
+    return c ? cudaGetErrorString(c->last_err) : "no context";
+}
+
+}  // extern "C"

@@ -1,0 +1,147 @@
+// Internal declarations shared by the CUDA translation units of libsph_b200.so.
+// (Nothing here is visible to, or shared with, oracle/.)
+#pragma once
+
+#include <cuda_runtime.h>
+#include <stdint.h>
+
+#include "sph.h"
+
+namespace sphb {
+
+constexpr int kRadixBits = 8;
+constexpr int kRadix = 1 << kRadixBits;
+constexpr int kMaxPasses = 4;
+
+// onesweep tile geometry
+constexpr int kSortThreads = 256;
+constexpr int kSortItems = 16;
+constexpr int kSortTile = kSortThreads * kSortItems;  // 4096 keys per tile
+
+// decoupled look-back status word: 2 flag bits + 30 value bits
+constexpr uint32_t kFlagAgg = 1u << 30;
+constexpr uint32_t kFlagPrefix = 2u << 30;
+constexpr uint32_t kFlagMask = 3u << 30;
+constexpr uint32_t kValueMask = ~kFlagMask;
+
+constexpr int kScanThreads = 256;
+constexpr int kScanItems = 8;
+constexpr int kScanTile = kScanThreads * kScanItems;
+
+struct Grid {
+    float ox, oy, oz;
+    float inv_edge;      // 1.0f / (2.0f * h), rounded once (reading S2)
+    int nx, ny, nz;
+    uint32_t n_cells;
+};
+
+struct Consts {
+    float support2;      // (2h)^2 in fp32
+    float half_inv_h;    // 0.5 / h
+    float cF;            // -(5 alpha / h^2),  alpha = 21 / (16 pi h^3)
+    float K, G;
+};
+
+struct Timing {
+    bool on = false;
+    cudaEvent_t ev[9] = {};
+};
+
+}  // namespace sphb
+
+struct sph_ctx {
+    sph_params params;
+    sphb::Grid grid;
+    sphb::Consts consts;
+    int64_t max_n;
+    cudaStream_t stream;
+    int device;
+    int num_sms;
+    int key_bits;        // live bits of the hash
+    int n_passes;
+    int64_t launches;
+    cudaError_t last_err;
+
+    // ---- scratch (device) ----
+    void *arena;                 // one allocation, carved below
+    size_t arena_bytes;
+    uint32_t *alt_keys, *alt_vals;            // radix ping-pong
+    uint32_t *hist;                           // [kMaxPasses][256] digit histograms -> exclusive
+    uint32_t *tile_status;                    // [passes][tiles][256]
+    uint32_t *tile_counter;                   // [kMaxPasses + 2] dynamic tile tickets
+    uint32_t *cell_mask;                      // [cells] owner bitmask per bucket
+    uint32_t *cell_flag_count;                // [cells] flagged particle count per bucket
+    uint32_t *cell_offset;                    // [cells] exclusive scan of the above
+    uint32_t *scan_status;                    // [scan tiles]
+    // step-internal products (used when the caller passes NULL)
+    uint32_t *s_hash, *s_sorted_hash, *s_perm, *s_cell_start, *s_cell_end, *s_comm_hash;
+    uint32_t *s_boundary_ids, *s_boundary_count, *s_owner_counts;
+    float *s_drho, *s_acc, *s_dsig[6];
+    unsigned long long *s_pair_count;
+    sph_state sorted;                         // sorted copy of the state
+    // host-API staging (lazy)
+    sph_state staging;
+    bool staging_ready;
+    sphb::Timing timing;
+};
+
+namespace sphb {
+
+#define SPH_CUDA_TRY(ctx, expr)                                  \
+    do {                                                         \
+        cudaError_t e__ = (expr);                                \
+        if (e__ != cudaSuccess) { (ctx)->last_err = e__; return SPH_ECUDA; } \
+    } while (0)
+
+#define SPH_CHECK_LAUNCH(ctx)                                    \
+    do {                                                         \
+        cudaError_t e__ = cudaPeekAtLastError();                 \
+        (ctx)->launches++;                                       \
+        if (e__ != cudaSuccess) { (ctx)->last_err = cudaGetLastError(); return SPH_ECUDA; } \
+    } while (0)
+
+static inline int div_up(int64_t a, int64_t b) { return (int)((a + b - 1) / b); }
+
+// stage launchers (each enqueues on ctx->stream, returns SPH_*)
+int launch_hash(sph_ctx *c, int64_t n, const float *posm, uint32_t *hash);
+int launch_sort(sph_ctx *c, int64_t n, const uint32_t *hash, uint32_t *sorted_hash, uint32_t *perm);
+int launch_reorder(sph_ctx *c, int64_t n, const uint32_t *perm, const sph_state *in,
+                   const sph_state *out);
+int launch_cell_ranges(sph_ctx *c, int64_t n, const uint32_t *sorted_hash, uint32_t *cs,
+                       uint32_t *ce);
+int launch_comm_hash(sph_ctx *c, int64_t n, const uint32_t *sorted_hash, const int32_t *sorted_owner,
+                     const uint32_t *perm, const uint32_t *cs, const uint32_t *ce,
+                     uint32_t *comm_hash, uint32_t *boundary_ids, uint32_t *boundary_count,
+                     uint32_t *owner_counts);
+int launch_interact(sph_ctx *c, int64_t n, const sph_state *sorted, const uint32_t *sorted_hash,
+                    const uint32_t *cs, const uint32_t *ce, float *drho, float *acc,
+                    float *const dsig[6], unsigned long long *pair_count);
+int launch_integrate(sph_ctx *c, int64_t n, float dt, const sph_state *in, const float *drho,
+                     const float *acc, const float *const dsig[6], const sph_state *out,
+                     const uint32_t *scatter_perm /* NULL = elementwise */);
+int launch_scan_exclusive(sph_ctx *c, int64_t n, const uint32_t *in, uint32_t *out,
+                          uint32_t *total /* dev scalar */);
+
+// ---- device helpers ----
+__device__ __forceinline__ uint32_t ld_volatile_u32(const uint32_t *p)
+{
+    uint32_t v;
+    asm volatile("ld.volatile.global.u32 %0, [%1];" : "=r"(v) : "l"(p) : "memory");
+    return v;
+}
+__device__ __forceinline__ void st_volatile_u32(uint32_t *p, uint32_t v)
+{
+    asm volatile("st.volatile.global.u32 [%0], %1;" ::"l"(p), "r"(v) : "memory");
+}
+__device__ __forceinline__ uint32_t lanemask_lt()
+{
+    uint32_t m;
+    asm("mov.u32 %0, %%lanemask_lt;" : "=r"(m));
+    return m;
+}
+__device__ __forceinline__ float4 ldg_f4(const float *p)
+{
+    return __ldg(reinterpret_cast<const float4 *>(p));
+}
+
+}  // namespace sphb
