@@ -234,7 +234,7 @@ static int step_impl(sph_ctx *c, int64_t n, float dt, const sph_state *state, ui
                      uint32_t *owner_counts, float *drho, float *acc, float *const dsig[6],
                      unsigned long long *pair_count, bool zero_pairs)
 {
-    if (!n_ok(c, n) || !state_ok(state)) return SPH_EINVAL;
+    if (!n_ok(c, n) || !state || (n > 0 && !state_ok(state))) return SPH_EINVAL;
     if (pair_count && zero_pairs)
         SPH_CUDA_TRY(c, cudaMemsetAsync(pair_count, 0, sizeof(unsigned long long), c->stream));
     if (!hash) hash = c->s_hash;

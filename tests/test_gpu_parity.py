@@ -1,0 +1,207 @@
+"""GPU parity tests (-m gpu): the CUDA path through the C-ABI binding vs the CPU oracle.
+
+Every case feeds the same seeded inputs (paper_2310_03596_b200.workloads) to both sides.
+Sizes span several onesweep tiles (4096 keys) with a ragged tail; the full-size configs are
+covered by tests/test_gpu_fullsize.py.
+"""
+import numpy as np
+import pytest
+import torch
+
+from paper_2310_03596_b200 import workloads as wl
+from tests import parity
+
+pytestmark = pytest.mark.gpu
+
+
+@pytest.fixture(scope="module")
+def sph():
+    if not torch.cuda.is_available():
+        pytest.fail("GPU tests need a CUDA device (no CPU fallback exists)")
+    from paper_2310_03596_b200 import sph as s
+    s.load_library()
+    return s
+
+
+# ------------------------------------------------------------------ whole step, lock-step parity
+@pytest.mark.parametrize("flags", [0, 1], ids=["tiled", "direct"])
+def test_cfg0_one_step(sph, oracle, flags):
+    w = wl.config(0)
+    rep = parity.lockstep(sph, oracle, w, steps=1, flags=flags)
+    assert 0 < rep[0]["boundary"] < w.n
+
+
+@pytest.mark.parametrize("flags", [0, 1], ids=["tiled", "direct"])
+def test_t1b_every_float_path(sph, oracle, flags):
+    w = wl.t1b()
+    rep = parity.lockstep(sph, oracle, w, steps=3, flags=flags)
+    assert rep[0]["pairs"] > 0
+
+
+@pytest.mark.parametrize("k,side,steps", [(1, 33, 3), (2, 37, 3), (4, 29, 2)])
+def test_scaled_configs(sph, oracle, k, side, steps):
+    w = wl.config(k, side=side)          # odd sides: ragged tiles everywhere
+    parity.lockstep(sph, oracle, w, steps=steps)
+
+
+def test_scaled_config3_clipped_geometry(sph, oracle):
+    w = wl.config(3, scale=0.1)          # plate + cylinders: long runs of empty buckets
+    assert w.n > 20000, w.n
+    parity.lockstep(sph, oracle, w, steps=2)
+
+
+def test_t1b_bigger_many_steps(sph, oracle):
+    w = wl.t1b(side=24, seed=1101)
+    parity.lockstep(sph, oracle, w, steps=5)
+
+
+# ------------------------------------------------------------------ degenerate cases
+def test_single_owner_has_no_boundary(sph, oracle):
+    w = wl.lattice_block(20, 20, 20, 0.1, 7, velocity=("normal", 0.05), owners=("single",))
+    rep = parity.lockstep(sph, oracle, w, steps=1)
+    assert rep[0]["boundary"] == 0
+
+
+def test_random_owners_everything_is_boundary(sph, oracle):
+    w = wl.lattice_block(20, 20, 20, 0.1, 8, velocity=("normal", 0.05), owners=("random", 16))
+    rep = parity.lockstep(sph, oracle, w, steps=1)
+    assert rep[0]["boundary"] == w.n
+
+
+def test_32_owners(sph, oracle):
+    w = wl.lattice_block(24, 20, 16, 0.1, 9, velocity=("normal", 0.05), owners=("random", 32))
+    parity.lockstep(sph, oracle, w, steps=1)
+
+
+def test_empty_and_tiny_inputs(sph, oracle):
+    w = wl.t1b(side=6)
+    for n in (0, 1, 2, 31, 33):
+        sub = wl.Workload("sub", w.posm[:n].copy(), w.velr[:n].copy(), w.sig[:, :n].copy(),
+                          w.owner[:n].copy(), w.origin, w.dims, n_owners=2)
+        ctx = sph.Context.for_workload(sub, max_n=64)
+        st = sph.State.from_numpy(sub.posm, sub.velr, sub.sig, sub.owner)
+        out = ctx.alloc_outputs(n)
+        ref = oracle.step(sub.posm, sub.velr, sub.sig, sub.owner, sub.origin, sub.dims, sub.h, sub.K,
+                          sub.G, 2, sub.dt)
+        ctx.sph_step(st, sub.dt, out)
+        torch.cuda.synchronize()
+        parity.compare_integers(out, ref, n)
+        if n:
+            parity.compare_rates(out, ref.rates)
+            parity.compare_state(st, ref)
+        ctx.close()
+
+
+def test_single_bucket_grid_and_clamping(sph, oracle):
+    # every particle far outside a 1x1x1 grid: clamped, zero sort passes
+    w = wl.t1b(side=5)
+    w.dims = np.array([1, 1, 1], np.int32)
+    parity.lockstep(sph, oracle, w, steps=1)
+    # a 2x3x2 grid with most particles clamped onto its border buckets
+    w = wl.t1b(side=7)
+    w.dims = np.array([2, 3, 2], np.int32)
+    w.origin = np.array([1.0, 0.5, 2.0], np.float32)
+    parity.lockstep(sph, oracle, w, steps=1)
+
+
+def test_coincident_particles(sph, oracle):
+    w = wl.t1b(side=8)
+    w.posm[1::7, :3] = w.posm[0::7, :3][: w.posm[1::7].shape[0]]   # exact duplicates (S15)
+    rep = parity.lockstep(sph, oracle, w, steps=1)
+    assert np.isfinite(rep[0]["acc"])
+
+
+def test_hash_at_bucket_faces(sph, oracle):
+    # positions exactly on, and one ulp either side of, bucket faces (reading S2)
+    h = np.float32(1.3)
+    edge = np.float32(2.0) * h
+    origin = np.array([-2.6, -2.6, -2.6], np.float32)
+    dims = np.array([9, 9, 9], np.int32)
+    faces = (np.arange(0, 9, dtype=np.float32) * edge + origin[0]).astype(np.float32)
+    xs = np.concatenate([faces, np.nextafter(faces, np.float32(1e9)), np.nextafter(faces, np.float32(-1e9)),
+                         np.array([-100.0, 100.0, 0.0, -0.0], np.float32)])
+    n = xs.shape[0]
+    posm = np.zeros((n, 4), np.float32)
+    posm[:, 0] = xs
+    posm[:, 1] = xs[::-1]
+    posm[:, 2] = np.roll(xs, 5)
+    ctx = sph.Context(origin, dims, h, max_n=n)
+    got = parity.u32(ctx.sph_hash(torch.from_numpy(posm).cuda()))
+    np.testing.assert_array_equal(got, oracle.hash(posm, origin, dims, h))
+    ctx.close()
+
+
+# ------------------------------------------------------------------ stage-by-stage C-ABI calls
+def test_stage_calls_match_oracle(sph, oracle):
+    w = wl.config(1, side=30)
+    ctx = sph.Context.for_workload(w)
+    st = sph.State.from_numpy(w.posm, w.velr, w.sig, w.owner)
+    ref = oracle.step(w.posm, w.velr, w.sig, w.owner, w.origin, w.dims, w.h, w.K, w.G, w.n_owners, w.dt)
+    hsh = ctx.sph_hash(st.posm)
+    sh, perm = ctx.sph_sort(hsh)
+    srt = ctx.sph_reorder(perm, st)
+    cs, ce = ctx.sph_cell_ranges(sh)
+    ch, bids, cnt, oc = ctx.sph_comm_hash(sh, srt.owner, perm, cs, ce)
+    drho, acc, dsig, pc = ctx.sph_interact(srt, sh, cs, ce)
+    new = ctx.sph_integrate(w.dt, srt, drho, acc, dsig)
+    torch.cuda.synchronize()
+    out = sph.StepOutputs(hsh, sh, perm, cs, ce, ch, bids, cnt, oc, drho, acc, dsig, pc)
+    parity.compare_integers(out, ref, w.n)
+    parity.compare_rates(out, ref.rates)
+    p = ref.perm.astype(np.int64)
+    np.testing.assert_array_equal(srt.posm.cpu().numpy(), w.posm[p])
+    np.testing.assert_array_equal(srt.velr.cpu().numpy(), w.velr[p])
+    np.testing.assert_array_equal(srt.sig.cpu().numpy(), w.sig[:, p])
+    np.testing.assert_array_equal(srt.owner.cpu().numpy(), w.owner[p])
+    # sph_integrate is elementwise (sorted order in, sorted order out)
+    assert parity.field_err(new.posm.cpu().numpy(), ref.posm[p]) <= parity.STATE_TOL
+    assert parity.field_err(new.velr.cpu().numpy(), ref.velr[p]) <= parity.STATE_TOL
+    assert parity.field_err(new.sig.cpu().numpy(), ref.sig[:, p]) <= parity.STATE_TOL
+    assert ctx.launch_count() > 0
+    ctx.close()
+
+
+def test_sort_random_keys_many_tiles(sph, oracle):
+    # sort alone on adversarial key distributions: uniform random, all equal, descending, two values
+    rng = np.random.default_rng(5)
+    dims = np.array([156, 156, 156], np.int32)     # 22 live bits, 3 passes
+    cells = int(np.prod(dims.astype(np.int64)))
+    n = 5 * 4096 + 1234
+    ctx = sph.Context(np.zeros(3, np.float32), dims, 1.3, max_n=n)
+    for keys in (rng.integers(0, cells, n), np.full(n, cells - 1), np.arange(n)[::-1] % cells,
+                 rng.integers(0, 2, n) * (cells - 1), rng.integers(0, 300, n)):
+        keys = keys.astype(np.uint32)
+        sh, perm = ctx.sph_sort(torch.from_numpy(keys.view(np.int32)).cuda())
+        rs, rp = oracle.sort(keys)
+        np.testing.assert_array_equal(parity.u32(sh), rs)
+        np.testing.assert_array_equal(parity.u32(perm), rp)
+    ctx.close()
+
+
+def test_step_host_end_to_end(sph, oracle):
+    w = wl.t1b(side=12)
+    ctx = sph.Context.for_workload(w)
+    host = sph.State.from_numpy(w.posm, w.velr, w.sig, w.owner, device="cpu", pin=True)
+    bids = np.zeros(w.n, np.uint32)
+    m, pairs = ctx.sph_step_host(host, w.dt, steps=1, boundary_ids=bids)
+    ref = oracle.step(w.posm, w.velr, w.sig, w.owner, w.origin, w.dims, w.h, w.K, w.G, w.n_owners, w.dt)
+    assert m == ref.boundary_ids.shape[0]
+    np.testing.assert_array_equal(bids[:m], ref.boundary_ids)
+    assert abs(pairs - ref.rates.pair_count) <= 2
+    parity.compare_state(host, ref)
+    ctx.close()
+
+
+def test_error_codes(sph):
+    with pytest.raises(sph.SphError):
+        sph.Context([0, 0, 0], [0, 1, 1], 1.3, max_n=10)
+    with pytest.raises(sph.SphError):
+        sph.Context([0, 0, 0], [4, 4, 4], -1.0, max_n=10)
+    with pytest.raises(sph.SphError):
+        sph.Context([0, 0, 0], [4, 4, 4], 1.3, n_owners=33, max_n=10)
+    with pytest.raises(sph.SphError):
+        sph.Context([0, 0, 0], [2048, 2048, 2048], 1.3, max_n=10)
+    ctx = sph.Context([0, 0, 0], [4, 4, 4], 1.3, max_n=8)
+    with pytest.raises(sph.SphError):
+        ctx.sph_hash(torch.zeros((9, 4), device="cuda"))       # n > max_n
+    ctx.close()
