@@ -20,42 +20,7 @@ interact_direct_kernel(int64_t n, InteractIn in, const uint32_t *__restrict__ so
     if (i < n) {
         const uint32_t h = sorted_hash[i];
         const int cx = h % g.nx, cy = (h / g.nx) % g.ny, cz = h / (g.nx * g.ny);
-        const float4 pi = in.posm[i];
-        const float4 vi = in.velr[i];
-        PairAccum A;
-        A.clear();
-        const int x0 = max(cx - 1, 0), x1 = min(cx + 1, g.nx - 1);
-        for (int dz = -1; dz <= 1; ++dz) {
-            const int z = cz + dz;
-            if (z < 0 || z >= g.nz) continue;
-            for (int dy = -1; dy <= 1; ++dy) {
-                const int y = cy + dy;
-                if (y < 0 || y >= g.ny) continue;
-                const uint32_t row = (uint32_t)g.nx * ((uint32_t)y + (uint32_t)g.ny * (uint32_t)z);
-                const uint32_t jb = cs[row + x0], je = ce[row + x1];
-                for (uint32_t j = jb; j < je; ++j) {
-                    const float4 pj = in.posm[j];
-                    const float dx = pi.x - pj.x, dy_ = pi.y - pj.y, dz_ = pi.z - pj.z;
-                    const float r2 = dx * dx + dy_ * dy_ + dz_ * dz_;
-                    if (r2 < k.support2 && j != (uint32_t)i) {
-                        const float4 vj = in.velr[j];
-                        const float inv_rho = 1.0f / vj.w;
-                        const float Vj = pj.w * inv_rho;
-                        const float ir2 = inv_rho * inv_rho;
-                        float Sj[6];
-#pragma unroll
-                        for (int c = 0; c < 6; ++c) Sj[c] = in.sig[c][j] * ir2;
-                        A.add(dx, dy_, dz_, r2, pj.w, Vj, vj.x - vi.x, vj.y - vi.y, vj.z - vi.z, Sj,
-                              k.half_inv_h);
-                        ++my_pairs;
-                    }
-                }
-            }
-        }
-        float si[6];
-#pragma unroll
-        for (int c = 0; c < 6; ++c) si[c] = in.sig[c][i];
-        finish_particle(A, si, vi.w, k, out, i);
+        my_pairs = direct_particle(i, cx, cy, cz, in, cs, ce, g, k, out);
     }
     if (pair_count) {
         // warp, then one atomic per warp

@@ -79,6 +79,8 @@ struct sph_ctx {
     float *s_drho, *s_acc, *s_dsig[6];
     unsigned long long *s_pair_count;
     sph_state sorted;                         // sorted copy of the state
+    float4 *rec_B, *rec_C;                    // packed neighbour records of the interaction kernel
+    float2 *rec_D;
     // host-API staging (lazy)
     sph_state staging;
     bool staging_ready;
