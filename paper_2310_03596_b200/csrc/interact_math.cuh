@@ -21,6 +21,14 @@ struct InteractOut {
     float *dsig[6];
 };
 
+// MUFU.RSQ without the denormal fix-up of rsqrtf (the argument is clamped to >= 1e-30 by the caller)
+__device__ __forceinline__ float rsqrt_approx(float x)
+{
+    float y;
+    asm("rsqrt.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x));
+    return y;
+}
+
 struct PairAccum {
     float dr;          // sum dv . mx
     float L[9];        // sum dv_a * wx_b
@@ -40,8 +48,8 @@ struct PairAccum {
                                         float half_inv_h)
     {
         const float r2c = fmaxf(r2, 1e-30f);          // coincident particles: gradW = 0 (S15)
-        const float r = r2c * rsqrtf(r2c);
-        const float t = fmaf(r, -half_inv_h, 1.0f);
+        const float r = r2c * rsqrt_approx(r2c);
+        const float t = fmaxf(fmaf(r, -half_inv_h, 1.0f), 0.0f);  // W = 0 beyond the support
         const float F = t * t * t;
         const float wm = mj * F, wV = Vj * F;
         const float mx = wm * dx, my = wm * dy, mz = wm * dz;
