@@ -217,7 +217,7 @@ def run_ours(args, rank, world, local_rank):
     for it in range(K):
         flush.zero_()                                   # L2 flush, outside the timed interval
         evs[it][0].record()
-        ctx.sph_step(state, w.dt, None, pair_acc)
+        ctx.sph_step(state, w.dt)                       # pair_count = NULL: the count is optional (include/sph.h)
         evs[it][1].record()
         if args.stage_timing:
             for k_, v in ctx.get_timing().items():

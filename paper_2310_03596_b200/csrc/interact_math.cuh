@@ -21,11 +21,11 @@ struct InteractOut {
     float *dsig[6];
 };
 
-// MUFU.RSQ without the denormal fix-up of rsqrtf (the argument is clamped to >= 1e-30 by the caller)
-__device__ __forceinline__ float rsqrt_approx(float x)
+// MUFU.SQRT: one instruction, sqrt(0) = 0 so coincident particles need no clamp (S15)
+__device__ __forceinline__ float sqrt_approx(float x)
 {
     float y;
-    asm("rsqrt.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x));
+    asm("sqrt.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x));
     return y;
 }
 
@@ -47,8 +47,7 @@ struct PairAccum {
                                         float dvx, float dvy, float dvz, const float (&S)[6],
                                         float half_inv_h)
     {
-        const float r2c = fmaxf(r2, 1e-30f);          // coincident particles: gradW = 0 (S15)
-        const float r = r2c * rsqrt_approx(r2c);
+        const float r = sqrt_approx(r2);              // coincident particles: r = 0, gradW = 0 (S15)
         const float t = fmaxf(fmaf(r, -half_inv_h, 1.0f), 0.0f);  // W = 0 beyond the support
         const float F = t * t * t;
         const float wm = mj * F, wV = Vj * F;
