@@ -1,7 +1,7 @@
 // Stage 2a: hand-written onesweep LSD radix sort on (hash, id)  (reading S5).
 //
 // One histogram kernel reads the keys once and builds the digit histograms of every pass.
-// Each pass is then ONE kernel: a tile of 4096 keys is ranked with warp-level match/popc
+// Each pass is then ONE kernel: a tile of 8192 keys is ranked with warp-level match/popc
 // (stable), the tile's per-digit counts are chained to the previous tiles with decoupled
 // look-back (single 32-bit status word = 2 flag bits + 30-bit count, so no fence is needed), and
 // keys/values are staged through shared memory so each digit's run leaves as one contiguous
@@ -35,13 +35,19 @@ __global__ void __launch_bounds__(256) radix_hist_kernel(int64_t n, const uint32
             for (int j = 0; j < cnt; ++j) k[j] = keys[base + j];
         }
         for (int p = 0; p < n_passes; ++p) {
+            uint32_t d[4];
 #pragma unroll
-            for (int j = 0; j < 4; ++j) {
-                // warp-aggregate equal digits (spatially coherent ids share their high digits)
-                const bool valid = j < cnt;
-                const uint32_t d = valid ? ((k[j] >> (p * kRadixBits)) & (kRadix - 1)) : 0x1000u;
-                const uint32_t peers = __match_any_sync(0xffffffffu, d);
-                if (valid && (peers & lanemask_lt()) == 0) atomicAdd(&s_hist[p][d], __popc(peers));
+            for (int j = 0; j < 4; ++j) d[j] = (k[j] >> (p * kRadixBits)) & (kRadix - 1);
+            // spatially coherent ids share their high digits: one atomic for the whole warp when
+            // all 128 keys agree, plain shared-memory atomics (few-way conflicts) otherwise
+            const uint32_t d0 = __shfl_sync(0xffffffffu, d[0], 0);
+            const bool same = cnt == 4 && d[0] == d0 && d[1] == d0 && d[2] == d0 && d[3] == d0;
+            if (__all_sync(0xffffffffu, same)) {
+                if ((threadIdx.x & 31) == 0) atomicAdd(&s_hist[p][d0], 128u);
+            } else {
+#pragma unroll
+                for (int j = 0; j < 4; ++j)
+                    if (j < cnt) atomicAdd(&s_hist[p][d[j]], 1u);
             }
         }
     }
@@ -73,27 +79,31 @@ __global__ void __launch_bounds__(kRadix) radix_hist_scan_kernel(uint32_t *hist)
 }
 
 // --------------------------------------------------------------------------- onesweep pass
+constexpr int kSortWarps = kSortThreads / 32;
+struct SortSmem {
+    uint32_t warp_hist[kSortWarps][kRadix];   // per-warp digit counts -> exclusive over the warps
+    uint32_t keys[kSortTile];
+    uint32_t vals[kSortTile];
+    uint32_t digit_base[kRadix];              // start of the digit's run inside the tile
+    uint32_t gbase[kRadix];                   // global position of that run minus digit_base
+    uint32_t scan[kRadix / 32];
+    uint32_t tile;
+};
+
 template <bool FIRST>
-__global__ void __launch_bounds__(kSortThreads)
+__global__ void __launch_bounds__(kSortThreads, 2)
 onesweep_kernel(int64_t n, const uint32_t *__restrict__ keys_in, const uint32_t *__restrict__ vals_in,
                 uint32_t *__restrict__ keys_out, uint32_t *__restrict__ vals_out,
                 const uint32_t *__restrict__ hist_excl, uint32_t *status, uint32_t *ticket, int shift)
 {
-    constexpr int kWarps = kSortThreads / 32;
-    __shared__ uint32_t s_warp_hist[kWarps][kRadix];
-    __shared__ uint32_t s_keys[kSortTile];
-    __shared__ uint32_t s_vals[kSortTile];
-    __shared__ uint32_t s_digit_base[kRadix];
-    __shared__ uint32_t s_gbase[kRadix];
-    __shared__ uint32_t s_scan[kWarps];
-    __shared__ uint32_t s_tile;
-
+    extern __shared__ __align__(16) unsigned char sort_smem_raw[];
+    SortSmem &sm = *reinterpret_cast<SortSmem *>(sort_smem_raw);
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
-    if (tid == 0) s_tile = atomicAdd(ticket, 1u);
+    if (tid == 0) sm.tile = atomicAdd(ticket, 1u);
 #pragma unroll
-    for (int i = tid; i < kWarps * kRadix; i += kSortThreads) (&s_warp_hist[0][0])[i] = 0;
+    for (int i = tid; i < kSortWarps * kRadix; i += kSortThreads) (&sm.warp_hist[0][0])[i] = 0;
     __syncthreads();
-    const uint32_t tile = s_tile;
+    const uint32_t tile = sm.tile;
     const int64_t tile_base = (int64_t)tile * kSortTile;
     const int tile_valid = (int)min((int64_t)kSortTile, n - tile_base);
     const int64_t chunk = tile_base + warp * (32 * kSortItems) + lane;
@@ -124,72 +134,86 @@ onesweep_kernel(int64_t n, const uint32_t *__restrict__ keys_in, const uint32_t 
         const uint32_t d = (key[r] >> shift) & (kRadix - 1);
         const uint32_t peers = __match_any_sync(0xffffffffu, d);
         const uint32_t before = __popc(peers & lt);
+        // the lowest peer books the whole group in the warp-private histogram; the atomics of
+        // successive rounds leave the warp in program order, so no __syncwarp is needed and the
+        // 16 rounds overlap
         uint32_t basev = 0;
-        if (before == 0) {
-            basev = s_warp_hist[warp][d];
-            s_warp_hist[warp][d] = basev + __popc(peers);
-        }
-        __syncwarp();
+        if (before == 0) basev = atomicAdd(&sm.warp_hist[warp][d], (uint32_t)__popc(peers));
         basev = __shfl_sync(0xffffffffu, basev, __ffs(peers) - 1);
         rank[r] = basev + before;
     }
     __syncthreads();
 
-    // ---- per-digit work: thread d owns digit d ----
-    {
-        const int d = tid;
-        uint32_t run = 0;
+    // ---- per-digit work: thread d < 256 owns digit d ----
+    const int d = tid;
+    uint32_t my_total = 0, run = 0, inc = 0;
+    if (d < kRadix) {
 #pragma unroll
-        for (int w = 0; w < kWarps; ++w) {
-            const uint32_t c = s_warp_hist[w][d];
-            s_warp_hist[w][d] = run;
+        for (int w = 0; w < kSortWarps; ++w) {
+            const uint32_t c = sm.warp_hist[w][d];
+            sm.warp_hist[w][d] = run;
             run += c;
         }
         // padding keys (0xFFFFFFFF) sit at the very end of digit 255
-        const uint32_t valid_total = (d == kRadix - 1) ? run - (uint32_t)(kSortTile - tile_valid) : run;
-        uint32_t *my_status = status + (size_t)tile * kRadix + d;
-        st_volatile_u32(my_status, (tile == 0 ? kFlagPrefix : kFlagAgg) | valid_total);
-
+        my_total = (d == kRadix - 1) ? run - (uint32_t)(kSortTile - tile_valid) : run;
+        st_volatile_u32(status + (size_t)tile * kRadix + d, (tile == 0 ? kFlagPrefix : kFlagAgg) | my_total);
         // block exclusive scan of `run` over digits -> position of the digit's run in the tile
-        uint32_t inc = run;
+        inc = run;
 #pragma unroll
         for (int o = 1; o < 32; o <<= 1) {
             uint32_t x = __shfl_up_sync(0xffffffffu, inc, o);
             if (lane >= o) inc += x;
         }
-        if (lane == 31) s_scan[warp] = inc;
-        __syncthreads();
+        if (lane == 31) sm.scan[warp] = inc;
+    }
+    __syncthreads();
+    if (d < kRadix) {
         uint32_t add = 0;
 #pragma unroll
-        for (int i = 0; i < kWarps; ++i) add += (i < warp) ? s_scan[i] : 0u;
-        const uint32_t dbase = inc - run + add;
-        s_digit_base[d] = dbase;
-
-        // decoupled look-back over the previous tiles
-        uint32_t excl = 0;
-        if (tile > 0) {
-            int64_t t = (int64_t)tile - 1;
-            while (true) {
-                const uint32_t s = ld_volatile_u32(status + (size_t)t * kRadix + d);
-                const uint32_t f = s & kFlagMask;
-                if (f == 0) continue;  // not published yet
-                excl += s & kValueMask;
-                if (f == kFlagPrefix) break;
-                --t;
-            }
-            st_volatile_u32(my_status, kFlagPrefix | (excl + valid_total));
-        }
-        s_gbase[d] = hist_excl[d] + excl - dbase;
+        for (int i = 0; i < kRadix / 32; ++i) add += (i < warp) ? sm.scan[i] : 0u;
+        sm.digit_base[d] = inc - run + add;
     }
     __syncthreads();
 
-    // ---- scatter into the tile-local sorted order ----
+    // ---- scatter into the tile-local sorted order (needs no global offset yet: the look-back
+    //      comes after it, which gives the preceding tiles time to publish their prefixes) ----
 #pragma unroll
     for (int r = 0; r < kSortItems; ++r) {
-        const uint32_t d = (key[r] >> shift) & (kRadix - 1);
-        const uint32_t pos = s_digit_base[d] + s_warp_hist[warp][d] + rank[r];
-        s_keys[pos] = key[r];
-        s_vals[pos] = val[r];
+        const uint32_t dg = (key[r] >> shift) & (kRadix - 1);
+        const uint32_t pos = sm.digit_base[dg] + sm.warp_hist[warp][dg] + rank[r];
+        sm.keys[pos] = key[r];
+        sm.vals[pos] = val[r];
+    }
+
+    // ---- decoupled look-back over the previous tiles ----
+    if (d < kRadix) {
+        uint32_t excl = 0;
+        if (tile > 0) {
+            // kLook status words are requested at once (independent loads), then consumed in
+            // order: a thread-serial walk would cost one L2 round trip per preceding tile
+            constexpr int kLook = 8;
+            int64_t t = (int64_t)tile - 1;
+            bool done = false;
+            while (!done) {
+                uint32_t sw[kLook];
+#pragma unroll
+                for (int j = 0; j < kLook; ++j)
+                    sw[j] = (t - j >= 0) ? ld_volatile_u32(status + (size_t)(t - j) * kRadix + d) : kFlagPrefix;
+                int used = 0;
+#pragma unroll
+                for (int j = 0; j < kLook; ++j) {
+                    const uint32_t f = sw[j] & kFlagMask;
+                    if (!done && used == j && f != 0) {
+                        excl += sw[j] & kValueMask;
+                        used = j + 1;
+                        if (f == kFlagPrefix) done = true;
+                    }
+                }
+                t -= used;  // an unpublished word stops the batch; it is polled again
+            }
+            st_volatile_u32(status + (size_t)tile * kRadix + d, kFlagPrefix | (excl + my_total));
+        }
+        sm.gbase[d] = hist_excl[d] + excl - sm.digit_base[d];
     }
     __syncthreads();
 
@@ -198,11 +222,11 @@ onesweep_kernel(int64_t n, const uint32_t *__restrict__ keys_in, const uint32_t 
     for (int k = 0; k < kSortItems; ++k) {
         const int p = tid + k * kSortThreads;
         if (p < tile_valid) {
-            const uint32_t kk = s_keys[p];
-            const uint32_t d = (kk >> shift) & (kRadix - 1);
-            const uint32_t dst = s_gbase[d] + (uint32_t)p;
+            const uint32_t kk = sm.keys[p];
+            const uint32_t dg = (kk >> shift) & (kRadix - 1);
+            const uint32_t dst = sm.gbase[dg] + (uint32_t)p;
             keys_out[dst] = kk;
-            vals_out[dst] = s_vals[p];
+            vals_out[dst] = sm.vals[p];
         }
     }
 }
@@ -236,6 +260,14 @@ int launch_sort(sph_ctx *c, int64_t n, const uint32_t *hash, uint32_t *sorted_ha
     radix_hist_scan_kernel<<<P, kRadix, 0, c->stream>>>(c->hist);
     SPH_CHECK_LAUNCH(c);
 
+    static bool attr_set = false;
+    if (!attr_set) {
+        SPH_CUDA_TRY(c, cudaFuncSetAttribute(onesweep_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                             (int)sizeof(SortSmem)));
+        SPH_CUDA_TRY(c, cudaFuncSetAttribute(onesweep_kernel<false>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                             (int)sizeof(SortSmem)));
+        attr_set = true;
+    }
     // the last pass must land in (sorted_hash, perm): alternate backwards from there
     const uint32_t *kin = hash, *vin = nullptr;
     for (int p = 0; p < P; ++p) {
@@ -244,11 +276,11 @@ int launch_sort(sph_ctx *c, int64_t n, const uint32_t *hash, uint32_t *sorted_ha
         uint32_t *vout = to_user ? perm : c->alt_vals;
         uint32_t *status = c->tile_status + (size_t)p * tiles * kRadix;
         if (p == 0)
-            onesweep_kernel<true><<<(unsigned)tiles, kSortThreads, 0, c->stream>>>(
+            onesweep_kernel<true><<<(unsigned)tiles, kSortThreads, sizeof(SortSmem), c->stream>>>(
                 n, kin, vin, kout, vout, c->hist + p * kRadix, status, c->tile_counter + p,
                 p * kRadixBits);
         else
-            onesweep_kernel<false><<<(unsigned)tiles, kSortThreads, 0, c->stream>>>(
+            onesweep_kernel<false><<<(unsigned)tiles, kSortThreads, sizeof(SortSmem), c->stream>>>(
                 n, kin, vin, kout, vout, c->hist + p * kRadix, status, c->tile_counter + p,
                 p * kRadixBits);
         SPH_CHECK_LAUNCH(c);
@@ -294,23 +326,32 @@ scan_exclusive_kernel(int64_t n, const uint32_t *__restrict__ in, uint32_t *__re
         add += (i < warp) ? w : 0u;
         tile_total += w;
     }
-    if (tid == 0) {
-        st_volatile_u32(status + tile, (tile == 0 ? kFlagPrefix : kFlagAgg) | tile_total);
+    if (warp == 0) {
+        // warp-parallel decoupled look-back: lane l inspects tile t0 - l; the window moves back by
+        // 32 tiles until it holds an inclusive prefix with every tile after it published
+        if (lane == 0) st_volatile_u32(status + tile, (tile == 0 ? kFlagPrefix : kFlagAgg) | tile_total);
         uint32_t excl = 0;
         if (tile > 0) {
-            int64_t t = (int64_t)tile - 1;
+            int64_t t0 = (int64_t)tile - 1;
             while (true) {
-                const uint32_t s = ld_volatile_u32(status + t);
+                const int64_t t = t0 - lane;
+                const uint32_t s = t >= 0 ? ld_volatile_u32(status + t) : kFlagPrefix;  // nothing before tile 0
                 const uint32_t f = s & kFlagMask;
-                if (f == 0) continue;
-                excl += s & kValueMask;
-                if (f == kFlagPrefix) break;
-                --t;
+                const uint32_t pref = __ballot_sync(0xffffffffu, f == kFlagPrefix);
+                const uint32_t unpub = __ballot_sync(0xffffffffu, f == 0);
+                const int fp = pref ? __ffs(pref) - 1 : 31;          // last lane that counts
+                const uint32_t need = 0xffffffffu >> (31 - fp);      // lanes 0 .. fp
+                if (unpub & need) continue;                          // not all published yet
+                excl += __reduce_add_sync(0xffffffffu, lane <= fp ? (s & kValueMask) : 0u);
+                if (pref) break;
+                t0 -= 32;
             }
-            st_volatile_u32(status + tile, kFlagPrefix | (excl + tile_total));
+            if (lane == 0) st_volatile_u32(status + tile, kFlagPrefix | (excl + tile_total));
         }
-        s_excl = excl;
-        if ((int64_t)(tile + 1) * kScanTile >= n && total_out) *total_out = excl + tile_total;
+        if (lane == 0) {
+            s_excl = excl;
+            if ((int64_t)(tile + 1) * kScanTile >= n && total_out) *total_out = excl + tile_total;
+        }
     }
     __syncthreads();
     uint32_t run = s_excl + add + (inc - sum);

@@ -14,9 +14,9 @@ constexpr int kRadix = 1 << kRadixBits;
 constexpr int kMaxPasses = 4;
 
 // onesweep tile geometry
-constexpr int kSortThreads = 256;
+constexpr int kSortThreads = 512;
 constexpr int kSortItems = 16;
-constexpr int kSortTile = kSortThreads * kSortItems;  // 4096 keys per tile
+constexpr int kSortTile = kSortThreads * kSortItems;  // 8192 keys per tile
 
 // decoupled look-back status word: 2 flag bits + 30 value bits
 constexpr uint32_t kFlagAgg = 1u << 30;
@@ -125,15 +125,17 @@ int launch_scan_exclusive(sph_ctx *c, int64_t n, const uint32_t *in, uint32_t *o
                           uint32_t *total /* dev scalar */);
 
 // ---- device helpers ----
+// look-back status words carry flag and value in ONE 32-bit word, so relaxed gpu-scope accesses
+// (served by L2) are enough; ld.volatile would be a system-scope load
 __device__ __forceinline__ uint32_t ld_volatile_u32(const uint32_t *p)
 {
     uint32_t v;
-    asm volatile("ld.volatile.global.u32 %0, [%1];" : "=r"(v) : "l"(p) : "memory");
+    asm volatile("ld.relaxed.gpu.global.u32 %0, [%1];" : "=r"(v) : "l"(p) : "memory");
     return v;
 }
 __device__ __forceinline__ void st_volatile_u32(uint32_t *p, uint32_t v)
 {
-    asm volatile("st.volatile.global.u32 [%0], %1;" ::"l"(p), "r"(v) : "memory");
+    asm volatile("st.relaxed.gpu.global.u32 [%0], %1;" ::"l"(p), "r"(v) : "memory");
 }
 __device__ __forceinline__ uint32_t lanemask_lt()
 {

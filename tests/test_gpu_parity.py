@@ -1,7 +1,7 @@
 """GPU parity tests (-m gpu): the CUDA path through the C-ABI binding vs the CPU oracle.
 
 Every case feeds the same seeded inputs (paper_2310_03596_b200.workloads) to both sides.
-Sizes span several onesweep tiles (4096 keys) with a ragged tail; the full-size configs are
+Sizes span several onesweep tiles (8192 keys) with a ragged tail; the full-size configs are
 covered by tests/test_gpu_fullsize.py.
 """
 import numpy as np
@@ -166,7 +166,7 @@ def test_sort_random_keys_many_tiles(sph, oracle):
     rng = np.random.default_rng(5)
     dims = np.array([156, 156, 156], np.int32)     # 22 live bits, 3 passes
     cells = int(np.prod(dims.astype(np.int64)))
-    n = 5 * 4096 + 1234
+    n = 5 * 8192 + 1234
     ctx = sph.Context(np.zeros(3, np.float32), dims, 1.3, max_n=n)
     for keys in (rng.integers(0, cells, n), np.full(n, cells - 1), np.arange(n)[::-1] % cells,
                  rng.integers(0, 2, n) * (cells - 1), rng.integers(0, 300, n)):
