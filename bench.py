@@ -118,6 +118,24 @@ def candidates_and_counts(cell_start, cell_end, dims):
     return int((cnt * box).sum())
 
 
+def max_over_ranks(x, world, device):
+    """Device-timed quantities are reported as the MAX over ranks (all-reduce on `device`:
+    NCCL on the GPU box, gloo in the CPU tests)."""
+    if world <= 1:
+        return float(x)
+    import torch
+    import torch.distributed as dist
+    t = torch.tensor([float(x)], dtype=torch.float64, device=device)
+    dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    return float(t.item())
+
+
+def whole_job_value(n_per_rank, steps, world, total_ms):
+    """Replicas only: every rank steps its own copy of the workload, so the
+    job processed world * n * steps particles in the slowest rank's time."""
+    return world * n_per_rank * steps / (total_ms * 1e-3)
+
+
 def oracle_sample(w, n_sample):
     """Bounded sample of the workload for the CPU legs: the first n_sample particles in id order
     (whole lattice planes from z = 0), on the workload's own grid."""
@@ -227,10 +245,7 @@ def run_ours(args, rank, world, local_rank):
     total_ms = sum(a.elapsed_time(b) for a, b in evs)
     if not args.stage_timing:                            # stage times of the last step only
         stage_ms = ctx.get_timing()
-    t = torch.tensor([total_ms], dtype=torch.float64, device=dev)
-    if world > 1:
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-    total_ms = float(t.item())
+    total_ms = max_over_ranks(total_ms, world, dev)
 
     # ---- end to end through the C-ABI with pinned host buffers ----
     host = sph.State.from_numpy(w.posm, w.velr, w.sig, w.owner, device="cpu", pin=True)
@@ -244,10 +259,7 @@ def run_ours(args, rank, world, local_rank):
         m_last, _pc = ctx.sph_step_host(host, w.dt, 1, bids)   # synchronises before returning
     torch.cuda.synchronize(dev)
     e2e_s = time.perf_counter() - t0
-    te = torch.tensor([e2e_s], dtype=torch.float64, device=dev)
-    if world > 1:
-        dist.all_reduce(te, op=dist.ReduceOp.MAX)
-    e2e_s = float(te.item())
+    e2e_s = max_over_ranks(e2e_s, world, dev)
     clocks = sampler.stop() if rank == 0 else None
     if rank != 0:
         return
@@ -255,7 +267,7 @@ def run_ours(args, rank, world, local_rank):
     peaks = load_peaks()
     props = torch.cuda.get_device_properties(dev)
     ms_per_step = total_ms / K
-    value = world * n * K / (total_ms * 1e-3)
+    value = whole_job_value(n, K, world, total_ms)
     flops = FLOP_PER_CAND * cand_step + FLOP_PER_PAIR * pairs_step
     t_int = stage_ms["interact"] * 1e-3
     fp32_peak = fp32_peak_tflops(props.multi_processor_count, peaks["sm_max_mhz"])
