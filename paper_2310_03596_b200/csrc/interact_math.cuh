@@ -64,6 +64,120 @@ struct PairAccum {
     }
 };
 
+// ---- packed fp32 pairs (sm_100a: FFMA2 / FADD2 / FMUL2, one issue slot for two lanes' worth of
+// fp32 work; a scalar operand is broadcast by the hardware, SASS `R.F32`) ------------------------
+typedef unsigned long long f32x2;
+__device__ __forceinline__ f32x2 pk(float lo, float hi)
+{
+    f32x2 r;
+    asm("mov.b64 %0, {%1, %2};" : "=l"(r) : "f"(lo), "f"(hi));
+    return r;
+}
+__device__ __forceinline__ f32x2 bc(float s) { return pk(s, s); }
+__device__ __forceinline__ float lo_of(f32x2 v)
+{
+    float a, b;
+    asm("mov.b64 {%0, %1}, %2;" : "=f"(a), "=f"(b) : "l"(v));
+    return a;
+}
+__device__ __forceinline__ float hi_of(f32x2 v)
+{
+    float a, b;
+    asm("mov.b64 {%0, %1}, %2;" : "=f"(a), "=f"(b) : "l"(v));
+    return b;
+}
+__device__ __forceinline__ f32x2 fma2(f32x2 a, f32x2 b, f32x2 c)
+{
+    f32x2 d;
+    asm("fma.rn.f32x2 %0, %1, %2, %3;" : "=l"(d) : "l"(a), "l"(b), "l"(c));
+    return d;
+}
+__device__ __forceinline__ f32x2 mul2(f32x2 a, f32x2 b)
+{
+    f32x2 d;
+    asm("mul.rn.f32x2 %0, %1, %2;" : "=l"(d) : "l"(a), "l"(b));
+    return d;
+}
+__device__ __forceinline__ f32x2 add2(f32x2 a, f32x2 b)
+{
+    f32x2 d;
+    asm("add.rn.f32x2 %0, %1, %2;" : "=l"(d) : "l"(a), "l"(b));
+    return d;
+}
+__device__ __forceinline__ f32x2 sub2(f32x2 a, f32x2 b)
+{
+    f32x2 d;
+    asm("sub.rn.f32x2 %0, %1, %2;" : "=l"(d) : "l"(a), "l"(b));
+    return d;
+}
+
+// The same sums as PairAccum, held as fp32 pairs so that one pair costs 30 issue slots instead
+// of 46 (the FMA pipe does the same work; the freed slots go to the loads and the bookkeeping).
+// Neighbour record (tiled kernel): A = x, y, z, |p|^2;  B = vx, vy, vz, Szz;
+// C = Sxx, Sxy, Sxy, Syy;  D = Sxz, Syz, m, V   with S = sigma / rho^2, V = m / rho.
+struct PairAccum2 {
+    f32x2 dr2;            // (sum dvx mx, sum dvy my)
+    float drz;            // sum dvz mz
+    f32x2 Lx, Ly, Lz;     // rows a = x, y, z of L, columns (x, y):  sum dv_a (wx, wy)
+    f32x2 Lc;             // column z of rows x, y:                 sum (dvx, dvy) wz
+    float Lzz;
+    f32x2 g2;             // (sum mx, sum my)
+    float gz;
+    f32x2 a2;             // (sum (S m)_x, sum (S m)_y)
+    f32x2 az2;            // (sum Sxz mx, sum Syz my)
+    float azz;            // sum Szz mz
+    __device__ __forceinline__ void clear()
+    {
+        dr2 = Lx = Ly = Lz = Lc = g2 = a2 = az2 = 0ull;
+        drz = Lzz = gz = azz = 0.f;
+    }
+    // tp = target position (tile-local), tv = target velocity; pa..pd = the neighbour record
+    __device__ __forceinline__ float add(f32x2 tpxy, float tpz, f32x2 tvxy, float tvz, const float4 &pa,
+                                         const float4 &pb, const float4 &pc, const float4 &pd,
+                                         float neg_half_inv_h)
+    {
+        const f32x2 dxy = sub2(tpxy, pk(pa.x, pa.y));
+        const float dz = tpz - pa.z;
+        const f32x2 sq = mul2(dxy, dxy);
+        const float r2 = fmaf(dz, dz, lo_of(sq)) + hi_of(sq);
+        const float r = sqrt_approx(r2);              // coincident particles: r = 0, gradW = 0 (S15)
+        const float t = fmaxf(fmaf(r, neg_half_inv_h, 1.0f), 0.0f);  // W = 0 beyond the support
+        const float F = t * t * t;
+        const f32x2 wmV = mul2(bc(F), pk(pd.z, pd.w));            // (m F, V F)
+        const f32x2 mxy = mul2(bc(lo_of(wmV)), dxy);              // m F (dx, dy)
+        const f32x2 wxy = mul2(bc(hi_of(wmV)), dxy);              // V F (dx, dy)
+        const f32x2 mwz = mul2(bc(dz), wmV);                      // (m F dz, V F dz)
+        const float mz = lo_of(mwz), wz = hi_of(mwz);
+        const f32x2 dvxy = sub2(pk(pb.x, pb.y), tvxy);
+        const float dvz = pb.z - tvz;
+        dr2 = fma2(dvxy, mxy, dr2);
+        drz = fmaf(dvz, mz, drz);
+        Lx = fma2(bc(lo_of(dvxy)), wxy, Lx);
+        Ly = fma2(bc(hi_of(dvxy)), wxy, Ly);
+        Lz = fma2(bc(dvz), wxy, Lz);
+        Lc = fma2(bc(wz), dvxy, Lc);
+        Lzz = fmaf(dvz, wz, Lzz);
+        g2 = add2(g2, mxy);
+        gz += mz;
+        a2 = fma2(bc(lo_of(mxy)), pk(pc.x, pc.y), a2);
+        a2 = fma2(bc(hi_of(mxy)), pk(pc.z, pc.w), a2);
+        a2 = fma2(bc(mz), pk(pd.x, pd.y), a2);
+        az2 = fma2(pk(pd.x, pd.y), mxy, az2);
+        azz = fmaf(pb.w, mz, azz);
+        return r2;
+    }
+    // unpack into the 16 sums of PairAccum (same order: dr, L[9] row-major, g[3], a[3])
+    __device__ __forceinline__ void unpack(float (&v)[16]) const
+    {
+        v[0] = lo_of(dr2) + hi_of(dr2) + drz;
+        v[1] = lo_of(Lx); v[2] = hi_of(Lx); v[3] = lo_of(Lc);
+        v[4] = lo_of(Ly); v[5] = hi_of(Ly); v[6] = hi_of(Lc);
+        v[7] = lo_of(Lz); v[8] = hi_of(Lz); v[9] = Lzz;
+        v[10] = lo_of(g2); v[11] = hi_of(g2); v[12] = gz;
+        v[13] = lo_of(a2); v[14] = hi_of(a2); v[15] = lo_of(az2) + hi_of(az2) + azz;
+    }
+};
+
 // Per-particle epilogue: scale by cF, add the S_i term, form the stress rate (O8) and store.
 __device__ __forceinline__ void finish_particle(const PairAccum &A, const float (&sig_i)[6],
                                                 float rho_i, const Consts &k, const InteractOut &out,

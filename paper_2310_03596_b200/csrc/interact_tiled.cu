@@ -6,28 +6,32 @@
 //  * x-fastest hashing makes the three buckets (cx-1, cx, cx+1) contiguous in the sorted arrays.
 //    A CTA owns a tile of kTBX x kTBY buckets of one z-layer; its candidate window is the
 //    3 (kTBY + 2) rows of kTBX + 2 buckets around it, i.e. 12 contiguous runs of the sorted arrays.
-//    The window's packed records (A = x,y,z,m; B = vx,vy,vz,V; C = Sxx,Syy,Szz,Sxy; D = Sxz,Syz
-//    with V = m/rho, S = sigma/rho^2, written by pack_kernel) are brought to shared memory with
-//    1-D TMA bulk copies (cp.async.bulk + mbarrier), no register staging.
+//    The window's packed records, four 16-byte parts per particle (A = x,y,z,m -> after the shift
+//    x',y',z',|p'|^2; B = vx,vy,vz,Szz; C = Sxx,Sxy,Sxy,Syy; D = Sxz,Syz,m,V with V = m/rho,
+//    S = sigma/rho^2; B, C, D written by pack_kernel in the pair layout of PairAccum2) are brought
+//    to shared memory with 1-D TMA bulk copies (cp.async.bulk + mbarrier), no register staging.
 //  * Warp b builds the candidate table of bucket b once: the 27-bucket stencil as shared-memory
 //    record offsets, every run padded so that (table position) == (record index) mod 8.
 //  * Work unit = 4 consecutive targets of one bucket, dealt round-robin to the 8 warps.
 //    Phase 1 (distance tests): lane l tests candidate 32 s + l of the table against the 4 targets
-//    held in registers (one 128-bit shared load per 128 tests, expanded-form test in tile-local
-//    coordinates) and records the outcome as one bit per target; 3 shuffles give quarter-warp q
-//    the complete mask of target q, lane t owning the table positions = t (mod 8).
-//  * Compaction: every lane pops its bits into the target's neighbour list in shared memory
-//    (positions from an 8-lane prefix sum), so the list is grouped by record index mod 8.
-//  * Phase 2 (pair arithmetic): lane t of the quarter walks list[t R .. (t + 1) R), R =
-//    ceil(len / 8): all lanes carry the same number of pairs (the v3 kernel ran at 61 % lane
-//    efficiency because a lane was tied to its residue class) and the 8 record gathers of a
-//    quarter-warp still fall mostly into 8 distinct 16-byte bank groups.  The 16 partial sums
-//    are reduced over the 8 lanes, parked in shared memory, and a lane-per-target epilogue forms
-//    the rates (O8) and stores them.
+//    held in registers as two fp32 pairs (one 128-bit shared load per 128 tests; expanded-form
+//    test in tile-local coordinates, 4 FFMA2 per 2 tests) and records the outcome as one bit per
+//    target; 3 shuffles give quarter-warp q the complete mask of target q, lane t owning the table
+//    positions = t (mod 8).  The whole table (up to 640 positions) is tested before one drain.
+//  * Phase 2 (pair arithmetic): lane t of quarter q pops the set bits of its own mask words and
+//    evaluates those pairs directly, two per round -- no neighbour list, no compaction pass.
+//    Because lane t only ever gathers records whose index is = t (mod 8), the 8 128-bit gathers
+//    of a quarter-warp always hit 8 distinct bank groups: the gathers are conflict-free by
+//    construction (the list-based v4 / v5 variants measured 7-8 wavefronts per gather
+//    instruction against the ideal 4, profiles/r01c).  The price is lane imbalance (the warp runs
+//    max-over-lanes rounds; idle lanes evaluate the dummy record of their class), paid on a pair
+//    body that is packed (PairAccum2: FFMA2 / FMUL2 / FADD2, 30 issue slots per pair instead
+//    of 46).  The 16 partial sums are reduced over the 8 lanes, parked in shared memory, and a
+//    lane-per-target epilogue forms the rates (O8) and stores them.
 //  * No pair is skipped or evaluated twice: the self pair is accepted like any other (it
 //    contributes exactly zero because x_ii = 0) and is subtracted from pair_count.
-// Tiles whose window does not fit the shared-memory budget, buckets whose table overflows and
-// targets with more than kListCap neighbours fall back to the direct walk.
+// Tiles whose window does not fit the shared-memory budget and buckets whose table overflows
+// fall back to the direct walk.
 #include "sph_internal.cuh"
 #include "interact_math.cuh"
 
@@ -38,27 +42,26 @@ constexpr int kNB = kTBX * kTBY;       // target buckets per tile
 constexpr int kRowsY = kTBY + 2;       // window rows along y
 constexpr int kRuns = 3 * kRowsY;      // contiguous runs of the window
 constexpr int kTW = 8;                 // warps per CTA (== kNB: warp b builds the table of bucket b)
-constexpr int kCap = 1472;             // window records held in shared memory
+constexpr int kCap = 1536;             // window records held in shared memory (64 B each)
 constexpr int kCandCap = 640;          // candidate-table entries per bucket
-constexpr int kDrain = 512;            // candidates per phase-1 / compaction round trip (16 x 32)
-constexpr int kListCap = 128;          // neighbour-list entries per target
 constexpr int kSlots = 8;              // targets parked per warp before the epilogue
 constexpr int kAccStride = 17;         // 16 sums + 1 pad word (bank-conflict free)
-constexpr int kDummy = kCap;           // record index of the far-away dummy candidate
+constexpr int kDummy = kCap;           // kDummy + c: far-away dummy candidate of bank class c = 0..7
 static_assert(kTW == kNB, "warp b builds the candidate table of bucket b");
-static_assert((kCap + 1) * 8 < 65536, "table entries are record index * 8 in 16 bits");
+static_assert((kCap + 8) * 16 < 65536 && kCap % 8 == 0, "table entries are record index * 16 in 16 bits");
+static_assert(kCandCap == 640, "three mask words cover 20 chunks of 32 table positions");
 
 struct Packed {
     const float4 *A;                   // sorted posm (x, y, z, m)
-    float4 *B;                         // vx, vy, vz, V = m / rho
-    float4 *C;                         // Sxx, Syy, Szz, Sxy     (S = sigma / rho^2)
-    float2 *D;                         // Sxz, Syz
+    float4 *B;                         // vx, vy, vz, Szz
+    float4 *C;                         // Sxx, Sxy, Sxy, Syy     (S = sigma / rho^2)
+    float4 *D;                         // Sxz, Syz, m, V
 };
 
 // ------------------------------------------------------------------------------------ pack
 __global__ void __launch_bounds__(256)
 pack_kernel(int64_t n, InteractIn in, float4 *__restrict__ B, float4 *__restrict__ C,
-            float2 *__restrict__ D)
+            float4 *__restrict__ D)
 {
     const int64_t k = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
     if (k >= n) return;
@@ -66,9 +69,10 @@ pack_kernel(int64_t n, InteractIn in, float4 *__restrict__ B, float4 *__restrict
     const float4 v = in.velr[k];
     const float inv_rho = 1.0f / v.w;
     const float ir2 = inv_rho * inv_rho;
-    B[k] = make_float4(v.x, v.y, v.z, m * inv_rho);
-    C[k] = make_float4(in.sig[0][k] * ir2, in.sig[1][k] * ir2, in.sig[2][k] * ir2, in.sig[3][k] * ir2);
-    D[k] = make_float2(in.sig[4][k] * ir2, in.sig[5][k] * ir2);
+    const float sxy = in.sig[3][k] * ir2;
+    B[k] = make_float4(v.x, v.y, v.z, in.sig[2][k] * ir2);
+    C[k] = make_float4(in.sig[0][k] * ir2, sxy, sxy, in.sig[1][k] * ir2);
+    D[k] = make_float4(in.sig[4][k] * ir2, in.sig[5][k] * ir2, m, m * inv_rho);
 }
 
 // ------------------------------------------------------------------------------------ PTX
@@ -111,14 +115,12 @@ __device__ __forceinline__ void tma_load_1d(void *dst, const void *src, uint32_t
 
 // ------------------------------------------------------------------------------------ smem
 struct __align__(16) TileSmem {
-    float4 A[kCap + 2];       // x - ox, y - oy, z - oz, m   (tile-local coordinates after the shift)
-    float4 B[kCap + 2];
-    float4 C[kCap + 2];
-    float2 D[kCap + 2];
-    float P2[kCap + 2];       // |p'|^2 of the shifted position
+    float4 A[kCap + 8];       // x - ox, y - oy, z - oz (tile-local coordinates), |p'|^2
+    float4 B[kCap + 8];
+    float4 C[kCap + 8];
+    float4 D[kCap + 8];
     float acc[kTW][kSlots][kAccStride];
-    uint16_t cand[kNB][kCandCap];      // record index * 8
-    uint16_t list[kTW][4][kListCap];   // record index * 8, per warp and quarter
+    uint16_t cand[kNB][kCandCap];      // record index * 16 (byte offset into A / B / C / D)
     int cand_len[kNB];        // padded table length (multiple of 32), -1 = overflow -> direct walk
     int bkt_nt[kNB];          // targets in bucket b
     int bkt_tsm[kNB];         // shared-memory record index of its first target
@@ -153,29 +155,24 @@ __device__ __forceinline__ void reduce8_transposed(float (&v)[16], int t)
     }
 }
 
-// One phase-1 test: sign bit of (|p'|^2 - 2 T'.p' - thr) shifted into the mask (1 = inside).
-__device__ __forceinline__ void test_push(uint32_t &mask, const float4 &pa, float p2, float ax, float ay,
-                                          float az, float thr)
+// Phase-1 tests of one candidate against two targets held as an fp32 pair:
+// acc = -thr + a . p' + |p'|^2 per target (a = -2 T', expanded form), the two sign bits are
+// shifted into the mask (1 = inside), the higher slot first.
+__device__ __forceinline__ void test_push2(uint32_t &mask, const float4 &pa, f32x2 ax, f32x2 ay, f32x2 az,
+                                           f32x2 nth)
 {
-    float acc = fmaf(ax, pa.x, p2);
-    acc = fmaf(ay, pa.y, acc);
-    acc = fmaf(az, pa.z, acc);
-    acc -= thr;
-    mask = __funnelshift_l(__float_as_uint(acc), mask, 1);
+    f32x2 acc = fma2(bc(pa.x), ax, nth);
+    acc = fma2(bc(pa.y), ay, acc);
+    acc = fma2(bc(pa.z), az, acc);
+    acc = add2(acc, bc(pa.w));
+    mask = __funnelshift_l(__float_as_uint(hi_of(acc)), mask, 1);
+    mask = __funnelshift_l(__float_as_uint(lo_of(acc)), mask, 1);
 }
 
-// byte-offset views of the record arrays (table and list entries are record index * 8)
-__device__ __forceinline__ float4 ld_rec16(const float4 *base, uint32_t e8)
+// byte-offset view of the record arrays (table entries are record index * 16)
+__device__ __forceinline__ float4 ld_rec(const float4 *base, uint32_t e16)
 {
-    return *reinterpret_cast<const float4 *>(reinterpret_cast<const char *>(base) + 2u * e8);
-}
-__device__ __forceinline__ float2 ld_rec8(const float2 *base, uint32_t e8)
-{
-    return *reinterpret_cast<const float2 *>(reinterpret_cast<const char *>(base) + e8);
-}
-__device__ __forceinline__ float ld_rec4(const float *base, uint32_t e8)
-{
-    return *reinterpret_cast<const float *>(reinterpret_cast<const char *>(base) + (e8 >> 1));
+    return *reinterpret_cast<const float4 *>(reinterpret_cast<const char *>(base) + e16);
 }
 
 template <bool kCount>
@@ -197,12 +194,12 @@ interact_tiled_kernel(Packed rec, InteractIn in, const uint32_t *__restrict__ cs
     const int ry = cy0 - 1 + (lane % kRowsY), rz = cz - 1 + (lane / kRowsY);
     const bool row_ok = lane < kRuns && ry >= 0 && ry < g.ny && rz >= 0 && rz < g.nz;
     const uint32_t rrow = row_ok ? (uint32_t)g.nx * ((uint32_t)ry + (uint32_t)g.ny * (uint32_t)rz) : 0u;
-    int run_lo = 0, run_len = 0;  // first sorted index copied (even) and number of records
+    int run_lo = 0, run_len = 0;  // first sorted index copied and number of records (16-byte parts)
     if (row_ok) {
         const int lo = (int)cs[rrow + max(cx0 - 1, 0)], hi = (int)ce[rrow + min(cx0 + nbx, g.nx - 1)];
-        if (hi > lo) { run_lo = lo & ~1; run_len = hi - run_lo; }
+        if (hi > lo) { run_lo = lo; run_len = hi - lo; }
     }
-    const int run_cnt = (run_len + 1) & ~1;  // even record count: keeps every offset 16-byte aligned
+    const int run_cnt = run_len;
     int run_off = run_cnt;                   // exclusive prefix over lanes 0..kRuns-1
 #pragma unroll
     for (int o = 1; o < 16; o <<= 1) {
@@ -239,14 +236,14 @@ interact_tiled_kernel(Packed rec, InteractIn in, const uint32_t *__restrict__ cs
     } else {
         __syncthreads();  // mbarrier initialised before the copies are issued against it
         if (warp == 0) {
-            const uint32_t bytes = __reduce_add_sync(0xffffffffu, (uint32_t)run_len * 48u + (uint32_t)run_cnt * 8u);
+            const uint32_t bytes = __reduce_add_sync(0xffffffffu, (uint32_t)run_len * 64u);
             if (lane == 0) mbar_expect_tx(&sm.bar, bytes);
             __syncwarp();
             if (run_len > 0) {
                 tma_load_1d(&sm.A[run_off], rec.A + run_lo, (uint32_t)run_len * 16u, &sm.bar);
                 tma_load_1d(&sm.B[run_off], rec.B + run_lo, (uint32_t)run_len * 16u, &sm.bar);
                 tma_load_1d(&sm.C[run_off], rec.C + run_lo, (uint32_t)run_len * 16u, &sm.bar);
-                tma_load_1d(&sm.D[run_off], rec.D + run_lo, (uint32_t)run_cnt * 8u, &sm.bar);
+                tma_load_1d(&sm.D[run_off], rec.D + run_lo, (uint32_t)run_len * 16u, &sm.bar);
             }
         }
         // ---- candidate table of bucket b: its 27-bucket stencil as record offsets, every run
@@ -280,17 +277,17 @@ interact_tiled_kernel(Packed rec, InteractIn in, const uint32_t *__restrict__ cs
                     const int pad = (s - W) & 7;
                     if (W + pad + len <= kCandCap - 32) {
                         uint16_t *cw = cand + W + pad + lane;
-                        const int e0 = (s + lane) * 8;
-                        if (lane < pad) cand[W + lane] = (uint16_t)(kDummy * 8);
+                        const int e0 = (s + lane) * 16;
+                        if (lane < pad) cand[W + lane] = (uint16_t)((kDummy + ((W + lane) & 7)) * 16);
                         if (lane < len) cw[0] = (uint16_t)e0;
-                        if (lane + 32 < len) cw[32] = (uint16_t)(e0 + 256);
-                        for (int o = lane + 64; o < len; o += 32) cw[o - lane] = (uint16_t)(e0 + 8 * (o - lane));
+                        if (lane + 32 < len) cw[32] = (uint16_t)(e0 + 512);
+                        for (int o = lane + 64; o < len; o += 32) cw[o - lane] = (uint16_t)(e0 + 16 * (o - lane));
                     }
                     W += pad + len;
                 }
                 const bool overflow = W > kCandCap - 32;
                 const int Wp = (W + 31) & ~31;
-                if (!overflow && W + lane < Wp) cand[W + lane] = (uint16_t)(kDummy * 8);
+                if (!overflow && W + lane < Wp) cand[W + lane] = (uint16_t)((kDummy + ((W + lane) & 7)) * 16);
                 if (lane == 0) sm.cand_len[warp] = overflow ? -1 : Wp;
             }
             // shared-memory index of the first target: it sits in window run rc
@@ -310,15 +307,14 @@ interact_tiled_kernel(Packed rec, InteractIn in, const uint32_t *__restrict__ cs
             for (int j = tid; j < total; j += kTW * 32) {
                 float4 pa = sm.A[j];
                 pa.x -= ox; pa.y -= oy; pa.z -= oz;
+                pa.w = pa.x * pa.x + pa.y * pa.y + pa.z * pa.z;   // the mass travels in D.z
                 sm.A[j] = pa;
-                sm.P2[j] = pa.x * pa.x + pa.y * pa.y + pa.z * pa.z;
             }
-            if (tid == 0) {
-                sm.A[kDummy] = make_float4(1e18f, 1e18f, 1e18f, 0.f);
-                sm.B[kDummy] = make_float4(0.f, 0.f, 0.f, 0.f);
-                sm.C[kDummy] = make_float4(0.f, 0.f, 0.f, 0.f);
-                sm.D[kDummy] = make_float2(0.f, 0.f);
-                sm.P2[kDummy] = 3e36f;
+            if (tid < 8) {
+                sm.A[kDummy + tid] = make_float4(1e18f, 1e18f, 1e18f, 3e36f);
+                sm.B[kDummy + tid] = make_float4(0.f, 0.f, 0.f, 0.f);
+                sm.C[kDummy + tid] = make_float4(0.f, 0.f, 0.f, 0.f);
+                sm.D[kDummy + tid] = make_float4(0.f, 0.f, 0.f, 0.f);
             }
         }
         __syncthreads();  // window shifted, tables and bucket records visible to every warp
@@ -348,7 +344,6 @@ interact_tiled_kernel(Packed rec, InteractIn in, const uint32_t *__restrict__ cs
 
         const int q = lane >> 3, t = lane & 7;
         float(*acc)[kAccStride] = sm.acc[warp];
-        uint16_t *lst = sm.list[warp][q];
         int parked = 0;
         for (int gi = warp; gi < NG; gi += kTW) {
             // bucket of work unit gi = number of buckets that end at or before it
@@ -361,143 +356,112 @@ interact_tiled_kernel(Packed rec, InteractIn in, const uint32_t *__restrict__ cs
             const uint16_t *cand = sm.cand[b];
 
             // quarter q works for target 4p + q; slot d of the phase-1 registers holds target
-            // 4p + (q ^ d):  a = -2 T', thr = support^2 - |T'|^2 + rounding margin
+            // 4p + (q ^ d):  a = -2 T', nth = -(support^2 - |T'|^2 + rounding margin)
             const int my_t = 4 * p + q;
             const bool my_valid = my_t < bnt;
             float4 tp = make_float4(0.f, 0.f, 0.f, 0.f);
-            float ax[4], ay[4], az[4], th[4];
-            ax[0] = ay[0] = az[0] = 0.f;
-            th[0] = -1.f;  // |p'|^2 >= 0 > -1: an absent target accepts nothing
+            float ax0 = 0.f, ay0 = 0.f, az0 = 0.f;
+            float nt0 = 1.f;  // |p'|^2 + 1 > 0: an absent target accepts nothing
             if (my_valid) {
                 tp = sm.A[tbase + my_t];
-                const float t2 = tp.x * tp.x + tp.y * tp.y + tp.z * tp.z;
-                ax[0] = -2.0f * tp.x; ay[0] = -2.0f * tp.y; az[0] = -2.0f * tp.z;
+                const float t2 = tp.w;
+                ax0 = -2.0f * tp.x; ay0 = -2.0f * tp.y; az0 = -2.0f * tp.z;
                 // margin >= 1e-6 (2|T'| + 2h)^2, the rounding bound of the expanded form
-                th[0] = k.support2 - t2 + 1e-6f * (8.0f * t2 + 3.0f * k.support2);
+                nt0 = t2 - k.support2 - 1e-6f * (8.0f * t2 + 3.0f * k.support2);
             }
-#pragma unroll
-            for (int d = 1; d < 4; ++d) {
-                ax[d] = __shfl_xor_sync(0xffffffffu, ax[0], 8 * d);
-                ay[d] = __shfl_xor_sync(0xffffffffu, ay[0], 8 * d);
-                az[d] = __shfl_xor_sync(0xffffffffu, az[0], 8 * d);
-                th[d] = __shfl_xor_sync(0xffffffffu, th[0], 8 * d);
-            }
-
-            // ---- phase 1 + compaction, kDrain table positions at a time -----------------------
-            int len = 0;          // entries in this quarter's list (uniform over its 8 lanes)
-            bool ovf = false;
-            for (int base = 0; base < Wp; base += kDrain) {
-                // bit 4 s + d of (lo | hi << 32) <- candidate chunk s, slot d
-                uint32_t lo = 0, hi = 0;
-                const int nch = min(kDrain, Wp - base) >> 5;
-                const uint16_t *cb = cand + base + lane;
-#pragma unroll 2
-                for (int s = nch - 1; s >= 8; --s) {
-                    const uint32_t e = cb[32 * s];
-                    const float4 pa = ld_rec16(sm.A, e);
-                    const float p2 = ld_rec4(sm.P2, e);
-                    test_push(hi, pa, p2, ax[3], ay[3], az[3], th[3]);
-                    test_push(hi, pa, p2, ax[2], ay[2], az[2], th[2]);
-                    test_push(hi, pa, p2, ax[1], ay[1], az[1], th[1]);
-                    test_push(hi, pa, p2, ax[0], ay[0], az[0], th[0]);
-                }
-#pragma unroll 2
-                for (int s = min(nch, 8) - 1; s >= 0; --s) {
-                    const uint32_t e = cb[32 * s];
-                    const float4 pa = ld_rec16(sm.A, e);
-                    const float p2 = ld_rec4(sm.P2, e);
-                    test_push(lo, pa, p2, ax[3], ay[3], az[3], th[3]);
-                    test_push(lo, pa, p2, ax[2], ay[2], az[2], th[2]);
-                    test_push(lo, pa, p2, ax[1], ay[1], az[1], th[1]);
-                    test_push(lo, pa, p2, ax[0], ay[0], az[0], th[0]);
-                }
-                // every quarter collects the bits of its own target: slot d of the lanes of
-                // quarter q ^ d.  Afterwards bit beta of lo <-> table position
-                // base + t + 8 (beta ^ q), of hi <-> the same + 256.
-                {
-                    const uint32_t l1 = __shfl_xor_sync(0xffffffffu, lo, 8), h1 = __shfl_xor_sync(0xffffffffu, hi, 8);
-                    const uint32_t l2 = __shfl_xor_sync(0xffffffffu, lo, 16), h2 = __shfl_xor_sync(0xffffffffu, hi, 16);
-                    const uint32_t l3 = __shfl_xor_sync(0xffffffffu, lo, 24), h3 = __shfl_xor_sync(0xffffffffu, hi, 24);
-                    lo = (lo & 0x11111111u) | (l1 & 0x22222222u) | (l2 & 0x44444444u) | (l3 & 0x88888888u);
-                    hi = (hi & 0x11111111u) | (h1 & 0x22222222u) | (h2 & 0x44444444u) | (h3 & 0x88888888u);
-                }
-                // ---- compaction: 8-lane prefix sum of the bit counts, then every lane pops its
-                //      bits into list[pos ..) -----------------------------------------------------
-                const int c = __popc(lo) + __popc(hi);
-                int inc = c;
-#pragma unroll
-                for (int o = 1; o < 8; o <<= 1) {
-                    const int x = __shfl_up_sync(0xffffffffu, inc, o, 8);
-                    if (t >= o) inc += x;
-                }
-                const int tot = __shfl_sync(0xffffffffu, inc, 7, 8);
-                if (__any_sync(0xffffffffu, len + tot > kListCap)) { ovf = true; break; }
-                uint16_t *lw = lst + (len + inc - c);
-                len += tot;
-                const uint16_t *cq = cand + base + t;
-                uint32_t w = lo, w2 = hi;
-                while (w | w2) {
-                    if (w == 0u) { w = w2; w2 = 0u; cq += 256; }
-                    const int beta = 31 - __clz(w);
-                    w ^= 1u << beta;
-                    *lw++ = cq[(beta ^ q) << 3];
-                }
-            }
-            __syncwarp();
-            if (ovf) {
-                // a target with more than kListCap neighbours (very dense spot): direct walk
-                if (lane < 4 && 4 * p + lane < bnt)
-                    my_pairs += direct_particle((int64_t)btb0 + 4 * p + lane, cx0 + b % kTBX, cy0 + b / kTBX, cz,
-                                                in, cs, ce, g, k, out);
-                continue;
+            f32x2 ax01, ay01, az01, nt01, ax23, ay23, az23, nt23;
+            {
+                const float ax1 = __shfl_xor_sync(0xffffffffu, ax0, 8), ay1 = __shfl_xor_sync(0xffffffffu, ay0, 8);
+                const float az1 = __shfl_xor_sync(0xffffffffu, az0, 8), nt1 = __shfl_xor_sync(0xffffffffu, nt0, 8);
+                ax01 = pk(ax0, ax1); ay01 = pk(ay0, ay1); az01 = pk(az0, az1); nt01 = pk(nt0, nt1);
+                // slots 2, 3 = slots 0, 1 of the lane 16 away
+                ax23 = __shfl_xor_sync(0xffffffffu, ax01, 16); ay23 = __shfl_xor_sync(0xffffffffu, ay01, 16);
+                az23 = __shfl_xor_sync(0xffffffffu, az01, 16); nt23 = __shfl_xor_sync(0xffffffffu, nt01, 16);
             }
 
-            // ---- phase 2: lane t walks list[t R .. (t + 1) R), two pairs per round; lanes past
-            //      the end evaluate the dummy record, which contributes exactly zero -------------
+            // ---- phase 1: the whole table, bit 4 s + d of mask word s / 8 <- chunk s, slot d ----
+            uint32_t m0 = 0, m1 = 0, m2 = 0;
+            const int nch = Wp >> 5;
+            const uint16_t *cb = cand + lane;
+#pragma unroll 1
+            for (int s = nch - 1; s >= 16; --s) {
+                const float4 pa = ld_rec(sm.A, cb[32 * s]);
+                test_push2(m2, pa, ax23, ay23, az23, nt23);
+                test_push2(m2, pa, ax01, ay01, az01, nt01);
+            }
+#pragma unroll 2
+            for (int s = min(nch, 16) - 1; s >= 8; --s) {
+                const float4 pa = ld_rec(sm.A, cb[32 * s]);
+                test_push2(m1, pa, ax23, ay23, az23, nt23);
+                test_push2(m1, pa, ax01, ay01, az01, nt01);
+            }
+#pragma unroll 2
+            for (int s = min(nch, 8) - 1; s >= 0; --s) {
+                const float4 pa = ld_rec(sm.A, cb[32 * s]);
+                test_push2(m0, pa, ax23, ay23, az23, nt23);
+                test_push2(m0, pa, ax01, ay01, az01, nt01);
+            }
+            // every quarter collects the bits of its own target: slot d of the lanes of quarter
+            // q ^ d.  Afterwards bit beta of word w <-> table position 256 w + t + 8 (beta ^ q).
+            {
+                const uint32_t a1 = __shfl_xor_sync(0xffffffffu, m0, 8), b1 = __shfl_xor_sync(0xffffffffu, m1, 8);
+                const uint32_t a2 = __shfl_xor_sync(0xffffffffu, m0, 16), b2 = __shfl_xor_sync(0xffffffffu, m1, 16);
+                const uint32_t a3 = __shfl_xor_sync(0xffffffffu, m0, 24), b3 = __shfl_xor_sync(0xffffffffu, m1, 24);
+                m0 = (m0 & 0x11111111u) | (a1 & 0x22222222u) | (a2 & 0x44444444u) | (a3 & 0x88888888u);
+                m1 = (m1 & 0x11111111u) | (b1 & 0x22222222u) | (b2 & 0x44444444u) | (b3 & 0x88888888u);
+                if (nch > 16) {  // warp-uniform
+                    const uint32_t c1 = __shfl_xor_sync(0xffffffffu, m2, 8), c2 = __shfl_xor_sync(0xffffffffu, m2, 16);
+                    const uint32_t c3 = __shfl_xor_sync(0xffffffffu, m2, 24);
+                    m2 = (m2 & 0x11111111u) | (c1 & 0x22222222u) | (c2 & 0x44444444u) | (c3 & 0x88888888u);
+                }
+            }
+            // ---- phase 2: lane t of quarter q owns the accepted candidates of target q whose record
+            //      index is = t (mod 8) and evaluates them straight from its mask words, two per
+            //      round.  The 8 gathers of a quarter-warp always fall into 8 distinct 16-byte bank
+            //      groups (conflict-free by construction); a lane that has run out of bits gathers
+            //      the dummy record of its own class, which contributes exactly zero. -------------
+            const int c = __popc(m0) + __popc(m1) + __popc(m2);
+            const int rounds = (int)__reduce_max_sync(0xffffffffu, (unsigned)((c + 1) >> 1));
             float4 tv = make_float4(0.f, 0.f, 0.f, 0.f);
             if (my_valid) tv = sm.B[tbase + my_t];
-            PairAccum S;
+            const f32x2 tpxy = pk(tp.x, tp.y), tvxy = pk(tv.x, tv.y);
+            PairAccum2 S;
             S.clear();
             {
-                const int R = (len + 7) >> 3;
-                int Rmax = max(R, __shfl_xor_sync(0xffffffffu, R, 8));
-                Rmax = max(Rmax, __shfl_xor_sync(0xffffffffu, Rmax, 16));
-                const int p0 = t * R;
-                const int mine = max(min(R, len - p0), 0);   // entries this lane owns
-                const uint16_t *lp = lst + p0;
-                auto eval = [&](uint32_t e) {
-                    const float4 pa = ld_rec16(sm.A, e);
-                    const float4 pb = ld_rec16(sm.B, e);
-                    const float4 pc = ld_rec16(sm.C, e);
-                    const float2 pd = ld_rec8(sm.D, e);
-                    const float dx = tp.x - pa.x, dy = tp.y - pa.y, dz = tp.z - pa.z;
-                    const float r2 = dx * dx + dy * dy + dz * dz;
-                    if (kCount && r2 < k.support2) ++my_pairs;  // exact test (phase 1 has a rounding margin)
-                    const float Sj[6] = {pc.x, pc.y, pc.z, pc.w, pd.x, pd.y};
-                    S.add(dx, dy, dz, r2, pa.w, pb.w, pb.x - tv.x, pb.y - tv.y, pb.z - tv.z, Sj, k.half_inv_h);
+                const char *cq = reinterpret_cast<const char *>(cand + t);
+                const uint32_t qx = (uint32_t)q << 4, dummy = (uint32_t)(kDummy + t) * 16u;
+                uint32_t w = m0, w1 = m1, w2 = m2;
+                auto pop = [&]() -> uint32_t {
+                    if (w == 0u) { w = w1; w1 = w2; w2 = 0u; cq += 512; }
+                    if (w == 0u) { w = w1; w1 = 0u; cq += 512; }
+                    uint32_t e = dummy;
+                    if (w != 0u) {
+                        const uint32_t beta = 31u - (uint32_t)__clz(w);
+                        w ^= 1u << beta;
+                        e = *reinterpret_cast<const uint16_t *>(cq + ((beta << 4) ^ qx));
+                    }
+                    return e;
                 };
-                int r = 0;
-                for (; r + 2 <= Rmax; r += 2) {
-                    uint32_t e0 = (uint32_t)kDummy * 8u, e1 = e0;
-                    if (r < mine) e0 = lp[r];
-                    if (r + 1 < mine) e1 = lp[r + 1];
+                auto eval = [&](uint32_t e) {
+                    const float4 pa = ld_rec(sm.A, e);
+                    const float4 pb = ld_rec(sm.B, e);
+                    const float4 pc = ld_rec(sm.C, e);
+                    const float4 pd = ld_rec(sm.D, e);
+                    const float r2 = S.add(tpxy, tp.z, tvxy, tv.z, pa, pb, pc, pd, -k.half_inv_h);
+                    if (kCount && r2 < k.support2) ++my_pairs;  // exact test (phase 1 has a rounding margin)
+                };
+#pragma unroll 1
+                for (int r = 0; r < rounds; ++r) {
+                    const uint32_t e0 = pop();
+                    const uint32_t e1 = pop();
                     eval(e0);
                     eval(e1);
-                }
-                if (r < Rmax) {
-                    uint32_t e0 = (uint32_t)kDummy * 8u;
-                    if (r < mine) e0 = lp[r];
-                    eval(e0);
                 }
             }
             // ---- reduce the 16 sums over the quarter, park them -------------------------------
             {
                 float v[16];
-                v[0] = S.dr;
-#pragma unroll
-                for (int c = 0; c < 9; ++c) v[1 + c] = S.L[c];
-#pragma unroll
-                for (int c = 0; c < 3; ++c) { v[10 + c] = S.g[c]; v[13 + c] = S.a[c]; }
+                S.unpack(v);
                 reduce8_transposed(v, t);
                 float *row = acc[parked * 4 + q];
                 const int idx = ((t & 4) << 1) + ((t & 2) << 1) + ((t & 1) << 1);

@@ -67,7 +67,7 @@ void carve(sph_ctx *c, char *base, size_t *total)
     c->sorted.owner = k.take<int32_t>(n);
     c->rec_B = k.take<float4>(n + 2);
     c->rec_C = k.take<float4>(n + 2);
-    c->rec_D = k.take<float2>(n + 2);
+    c->rec_D = k.take<float4>(n + 2);
     *total = align_up(k.off, 256);
 }
 

@@ -80,7 +80,7 @@ struct sph_ctx {
     unsigned long long *s_pair_count;
     sph_state sorted;                         // sorted copy of the state
     float4 *rec_B, *rec_C;                    // packed neighbour records of the interaction kernel
-    float2 *rec_D;
+    float4 *rec_D;
     // host-API staging (lazy)
     sph_state staging;
     bool staging_ready;
