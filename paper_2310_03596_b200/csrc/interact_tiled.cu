@@ -428,17 +428,27 @@ interact_tiled_kernel(Packed rec, InteractIn in, const uint32_t *__restrict__ cs
             PairAccum2 S;
             S.clear();
             {
-                const char *cq = reinterpret_cast<const char *>(cand + t);
-                const uint32_t qx = (uint32_t)q << 4, dummy = (uint32_t)(kDummy + t) * 16u;
+                // three (mask word, table base) pairs, the non-empty words first; pop() is
+                // branch-free: refill the head word when it has run dry, take its highest bit
+                const uint32_t dummy = (uint32_t)(kDummy + t) * 16u;
+                const uint32_t cbase = smem_u32(cand + t);
                 uint32_t w = m0, w1 = m1, w2 = m2;
+                uint32_t c0 = cbase, c1 = cbase + 512u, c2 = cbase + 1024u;
+                if (w1 == 0u) { w1 = w2; c1 = c2; w2 = 0u; }
+                if (w == 0u) { w = w1; c0 = c1; w1 = w2; c1 = c2; w2 = 0u; }
                 auto pop = [&]() -> uint32_t {
-                    if (w == 0u) { w = w1; w1 = w2; w2 = 0u; cq += 512; }
-                    if (w == 0u) { w = w1; w1 = 0u; cq += 512; }
+                    const bool z = (w == 0u);
+                    w = z ? w1 : w;   c0 = z ? c1 : c0;
+                    w1 = z ? w2 : w1; c1 = z ? c2 : c1;
+                    w2 = z ? 0u : w2;
+                    const uint32_t beta = 31u - (uint32_t)__clz(w);   // 0xffffffff when w == 0
+                    const bool valid = (w != 0u);
+                    w &= ~(1u << (beta & 31u));
                     uint32_t e = dummy;
-                    if (w != 0u) {
-                        const uint32_t beta = 31u - (uint32_t)__clz(w);
-                        w ^= 1u << beta;
-                        e = *reinterpret_cast<const uint16_t *>(cq + ((beta << 4) ^ qx));
+                    if (valid) {
+                        uint16_t v;
+                        asm volatile("ld.shared.u16 %0, [%1];" : "=h"(v) : "r"(c0 + ((beta ^ (uint32_t)q) << 4)));
+                        e = v;
                     }
                     return e;
                 };
