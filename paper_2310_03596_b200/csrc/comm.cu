@@ -85,7 +85,7 @@ stencil_flag_kernel(Grid g, const uint32_t *__restrict__ cell_mask, const uint32
     flag_count[c] = (__popc(m) >= 2) ? (ce[c] - cs[c]) : 0u;
 }
 
-constexpr int kCompItems = 4;  // sorted particles per thread (128-bit loads and stores)
+constexpr int kCompItems = 8;  // sorted particles per thread (two 128-bit loads per array in flight)
 
 __global__ void __launch_bounds__(256)
 comm_hash_compact_kernel(int64_t n, const uint32_t *__restrict__ sorted_hash,
@@ -105,12 +105,15 @@ comm_hash_compact_kernel(int64_t n, const uint32_t *__restrict__ sorted_hash,
     const bool vec = full && ((reinterpret_cast<uintptr_t>(sorted_hash) | reinterpret_cast<uintptr_t>(sorted_owner) |
                                reinterpret_cast<uintptr_t>(perm) | reinterpret_cast<uintptr_t>(comm_hash)) & 15) == 0;
     if (vec) {
-        const uint4 a = __ldcs(reinterpret_cast<const uint4 *>(sorted_hash + k0));
-        const uint4 b = __ldcs(reinterpret_cast<const uint4 *>(perm + k0));
-        const int4 c = __ldcs(reinterpret_cast<const int4 *>(sorted_owner + k0));
-        h[0] = a.x; h[1] = a.y; h[2] = a.z; h[3] = a.w;
-        id[0] = b.x; id[1] = b.y; id[2] = b.z; id[3] = b.w;
-        o[0] = c.x; o[1] = c.y; o[2] = c.z; o[3] = c.w;
+#pragma unroll
+        for (int v = 0; v < kCompItems / 4; ++v) {
+            const uint4 a = __ldcs(reinterpret_cast<const uint4 *>(sorted_hash + k0) + v);
+            const uint4 b = __ldcs(reinterpret_cast<const uint4 *>(perm + k0) + v);
+            const int4 c = __ldcs(reinterpret_cast<const int4 *>(sorted_owner + k0) + v);
+            h[4 * v] = a.x; h[4 * v + 1] = a.y; h[4 * v + 2] = a.z; h[4 * v + 3] = a.w;
+            id[4 * v] = b.x; id[4 * v + 1] = b.y; id[4 * v + 2] = b.z; id[4 * v + 3] = b.w;
+            o[4 * v] = c.x; o[4 * v + 1] = c.y; o[4 * v + 2] = c.z; o[4 * v + 3] = c.w;
+        }
     } else {
 #pragma unroll
         for (int j = 0; j < kCompItems; ++j) {
@@ -120,8 +123,13 @@ comm_hash_compact_kernel(int64_t n, const uint32_t *__restrict__ sorted_hash,
             o[j] = ok ? sorted_owner[k0 + j] : 0;
         }
     }
-    // bucket records are fetched once per run of equal hashes
-    uint32_t ch[kCompItems];
+    // bucket records of the first and the last bucket of the thread are requested up front
+    // (independent loads); buckets in between (rare: 8 particles span 1-2 buckets) on demand
+    const uint32_t hf = h[0], hl = h[kCompItems - 1];
+    uint32_t fc_f = 0, off_f = 0, cs_f = 0, fc_l = 0, off_l = 0, cs_l = 0;
+    if (hf != 0xFFFFFFFFu) { fc_f = __ldg(flag_count + hf); off_f = __ldg(cell_offset + hf); cs_f = __ldg(cs + hf); }
+    if (hl != 0xFFFFFFFFu) { fc_l = __ldg(flag_count + hl); off_l = __ldg(cell_offset + hl); cs_l = __ldg(cs + hl); }
+    uint32_t ch[kCompItems], dst[kCompItems];
     uint32_t cur = 0xFFFFFFFFu, delta = 0u;   // delta = cell_offset - cell_start of a flagged bucket
     bool flagged = false;
     uint32_t my_owner = 0xFFu, my_cnt = 0u;   // flagged particles of this thread with owner my_owner
@@ -130,21 +138,44 @@ comm_hash_compact_kernel(int64_t n, const uint32_t *__restrict__ sorted_hash,
         if (h[j] != cur) {
             cur = h[j];
             flagged = false;
-            if (cur != 0xFFFFFFFFu && k0 + j < n) {
-                flagged = __ldg(flag_count + cur) != 0u;
-                if (flagged) delta = __ldg(cell_offset + cur) - __ldg(cs + cur);
+            if (cur != 0xFFFFFFFFu) {
+                uint32_t fc, of, c0;
+                if (cur == hf) { fc = fc_f; of = off_f; c0 = cs_f; }
+                else if (cur == hl) { fc = fc_l; of = off_l; c0 = cs_l; }
+                else { fc = __ldg(flag_count + cur); of = __ldg(cell_offset + cur); c0 = __ldg(cs + cur); }
+                flagged = fc != 0u;
+                delta = of - c0;
             }
         }
         ch[j] = flagged ? cur : SPH_GARBAGE_HASH;
+        dst[j] = flagged ? delta + (uint32_t)(k0 + j) : 0xFFFFFFFFu;
         if (flagged) {
-            boundary_ids[delta + (uint32_t)(k0 + j)] = id[j];
             const uint32_t oo = (uint32_t)o[j] & 31u;
             if (my_cnt == 0u) my_owner = oo;
             if (oo == my_owner) ++my_cnt; else atomicAdd(&s_cnt[oo], 1u);
         }
     }
+    // boundary ids: 128-bit stores where 4 consecutive slots are flagged, contiguous and aligned
+#pragma unroll
+    for (int v = 0; v < kCompItems / 4; ++v) {
+        const uint32_t d0 = dst[4 * v];
+        const bool run4 = d0 != 0xFFFFFFFFu && (d0 & 3u) == 0u && dst[4 * v + 1] == d0 + 1u &&
+                          dst[4 * v + 2] == d0 + 2u && dst[4 * v + 3] == d0 + 3u &&
+                          (reinterpret_cast<uintptr_t>(boundary_ids) & 15) == 0;
+        if (run4) {
+            __stcs(reinterpret_cast<uint4 *>(boundary_ids + d0),
+                   make_uint4(id[4 * v], id[4 * v + 1], id[4 * v + 2], id[4 * v + 3]));
+        } else {
+#pragma unroll
+            for (int j = 4 * v; j < 4 * v + 4; ++j)
+                if (dst[j] != 0xFFFFFFFFu) boundary_ids[dst[j]] = id[j];
+        }
+    }
     if (vec) {
-        __stcs(reinterpret_cast<uint4 *>(comm_hash + k0), make_uint4(ch[0], ch[1], ch[2], ch[3]));
+#pragma unroll
+        for (int v = 0; v < kCompItems / 4; ++v)
+            __stcs(reinterpret_cast<uint4 *>(comm_hash + k0) + v,
+                   make_uint4(ch[4 * v], ch[4 * v + 1], ch[4 * v + 2], ch[4 * v + 3]));
     } else {
 #pragma unroll
         for (int j = 0; j < kCompItems; ++j)

@@ -14,45 +14,79 @@
 namespace sphb {
 
 // --------------------------------------------------------------------------- histograms
+// Digit counts of one 128-bit load (4 consecutive keys of one thread) for pass P.  Spatially
+// coherent ids share their high digits: one atomic for the whole warp when all 128 keys agree,
+// one per thread when its 4 keys agree, 4 otherwise.
+template <int P>
+__device__ __forceinline__ void hist_add4(uint32_t (*s_hist)[kRadix], const uint4 &v, int lane)
+{
+    const uint32_t d0 = (v.x >> (P * kRadixBits)) & (kRadix - 1), d1 = (v.y >> (P * kRadixBits)) & (kRadix - 1);
+    const uint32_t d2 = (v.z >> (P * kRadixBits)) & (kRadix - 1), d3 = (v.w >> (P * kRadixBits)) & (kRadix - 1);
+    if (P == 0) {  // the lowest digit changes every few keys: no aggregation pays
+        atomicAdd(&s_hist[P][d0], 1u); atomicAdd(&s_hist[P][d1], 1u);
+        atomicAdd(&s_hist[P][d2], 1u); atomicAdd(&s_hist[P][d3], 1u);
+        return;
+    }
+    const bool same = (d0 == d1) & (d2 == d3) & (d0 == d2);
+    int all_lanes = 0;
+    __match_all_sync(0xffffffffu, same ? d0 : (0x100u + (uint32_t)lane), &all_lanes);
+    if (all_lanes) {
+        if (lane == 0) atomicAdd(&s_hist[P][d0], 128u);
+    } else if (same) {
+        atomicAdd(&s_hist[P][d0], 4u);
+    } else {
+        atomicAdd(&s_hist[P][d0], 1u); atomicAdd(&s_hist[P][d1], 1u);
+        atomicAdd(&s_hist[P][d2], 1u); atomicAdd(&s_hist[P][d3], 1u);
+    }
+}
+
+template <int NP>
 __global__ void __launch_bounds__(256) radix_hist_kernel(int64_t n, const uint32_t *__restrict__ keys,
-                                                         uint32_t *__restrict__ hist, int n_passes)
+                                                         uint32_t *__restrict__ hist)
 {
     __shared__ uint32_t s_hist[kMaxPasses][kRadix];
     for (int i = threadIdx.x; i < kMaxPasses * kRadix; i += blockDim.x) (&s_hist[0][0])[i] = 0;
     __syncthreads();
-    const int64_t stride = (int64_t)gridDim.x * blockDim.x * 4;
-    // block-uniform trip count, so every warp-collective below runs with a full mask
-    for (int64_t tb = (int64_t)blockIdx.x * blockDim.x * 4; tb < n; tb += stride) {
-        const int64_t base = tb + (int64_t)threadIdx.x * 4;
-        uint32_t k[4] = {0, 0, 0, 0};
-        int cnt = 0;
-        if (base + 4 <= n) {
-            uint4 v = __ldcs(reinterpret_cast<const uint4 *>(keys + base));
-            k[0] = v.x; k[1] = v.y; k[2] = v.z; k[3] = v.w;
-            cnt = 4;
-        } else if (base < n) {
-            cnt = (int)(n - base);
-            for (int j = 0; j < cnt; ++j) k[j] = keys[base + j];
+    const int lane = threadIdx.x & 31;
+    const int64_t n4 = n >> 2;                       // whole 128-bit groups
+    const int64_t stride = (int64_t)gridDim.x * blockDim.x;
+    // block-uniform trip count (the warp-collective needs full warps), two loads in flight
+    const int64_t iters = (n4 + 2 * stride - 1) / (2 * stride);
+    int64_t g = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    const uint4 *k4 = reinterpret_cast<const uint4 *>(keys);
+    for (int64_t it = 0; it < iters; ++it, g += 2 * stride) {
+        const bool ok0 = g < n4, ok1 = g + stride < n4;
+        uint4 a = make_uint4(0, 0, 0, 0), b = a;
+        if (ok0) a = __ldcs(k4 + g);
+        if (ok1) b = __ldcs(k4 + g + stride);
+        // a lane without data joins the collectives with a value that never matches
+        if (__all_sync(0xffffffffu, ok0)) {
+            hist_add4<0>(s_hist, a, lane);
+            if (NP > 1) hist_add4<1>(s_hist, a, lane);
+            if (NP > 2) hist_add4<2>(s_hist, a, lane);
+            if (NP > 3) hist_add4<3>(s_hist, a, lane);
+        } else if (ok0) {
+            const uint32_t kk[4] = {a.x, a.y, a.z, a.w};
+            for (int p = 0; p < NP; ++p)
+                for (int j = 0; j < 4; ++j) atomicAdd(&s_hist[p][(kk[j] >> (p * kRadixBits)) & (kRadix - 1)], 1u);
         }
-        for (int p = 0; p < n_passes; ++p) {
-            uint32_t d[4];
-#pragma unroll
-            for (int j = 0; j < 4; ++j) d[j] = (k[j] >> (p * kRadixBits)) & (kRadix - 1);
-            // spatially coherent ids share their high digits: one atomic for the whole warp when
-            // all 128 keys agree, plain shared-memory atomics (few-way conflicts) otherwise
-            const uint32_t d0 = __shfl_sync(0xffffffffu, d[0], 0);
-            const bool same = cnt == 4 && d[0] == d0 && d[1] == d0 && d[2] == d0 && d[3] == d0;
-            if (__all_sync(0xffffffffu, same)) {
-                if ((threadIdx.x & 31) == 0) atomicAdd(&s_hist[p][d0], 128u);
-            } else {
-#pragma unroll
-                for (int j = 0; j < 4; ++j)
-                    if (j < cnt) atomicAdd(&s_hist[p][d[j]], 1u);
-            }
+        if (__all_sync(0xffffffffu, ok1)) {
+            hist_add4<0>(s_hist, b, lane);
+            if (NP > 1) hist_add4<1>(s_hist, b, lane);
+            if (NP > 2) hist_add4<2>(s_hist, b, lane);
+            if (NP > 3) hist_add4<3>(s_hist, b, lane);
+        } else if (ok1) {
+            const uint32_t kk[4] = {b.x, b.y, b.z, b.w};
+            for (int p = 0; p < NP; ++p)
+                for (int j = 0; j < 4; ++j) atomicAdd(&s_hist[p][(kk[j] >> (p * kRadixBits)) & (kRadix - 1)], 1u);
         }
     }
+    // the ragged tail (n % 4 keys) goes to one thread
+    if (blockIdx.x == 0 && threadIdx.x == 0)
+        for (int64_t i = n4 << 2; i < n; ++i)
+            for (int p = 0; p < NP; ++p) atomicAdd(&s_hist[p][(keys[i] >> (p * kRadixBits)) & (kRadix - 1)], 1u);
     __syncthreads();
-    for (int i = threadIdx.x; i < n_passes * kRadix; i += blockDim.x) {
+    for (int i = threadIdx.x; i < NP * kRadix; i += blockDim.x) {
         uint32_t v = (&s_hist[0][0])[i];
         if (v) atomicAdd(hist + i, v);
     }
@@ -134,11 +168,14 @@ onesweep_kernel(int64_t n, const uint32_t *__restrict__ keys_in, const uint32_t 
         const uint32_t d = (key[r] >> shift) & (kRadix - 1);
         const uint32_t peers = __match_any_sync(0xffffffffu, d);
         const uint32_t before = __popc(peers & lt);
-        // the lowest peer books the whole group in the warp-private histogram; the atomics of
-        // successive rounds leave the warp in program order, so no __syncwarp is needed and the
-        // 16 rounds overlap
         uint32_t basev = 0;
-        if (before == 0) basev = atomicAdd(&sm.warp_hist[warp][d], (uint32_t)__popc(peers));
+        // the histogram is private to the warp: the lowest peer books the whole group with a plain
+        // read-modify-write (shared-memory atomics with a return value measured slower)
+        if (before == 0) {
+            basev = sm.warp_hist[warp][d];
+            sm.warp_hist[warp][d] = basev + (uint32_t)__popc(peers);
+        }
+        __syncwarp();
         basev = __shfl_sync(0xffffffffu, basev, __ffs(peers) - 1);
         rank[r] = basev + before;
     }
@@ -255,7 +292,12 @@ int launch_sort(sph_ctx *c, int64_t n, const uint32_t *hash, uint32_t *sorted_ha
                                     c->stream));
     int hb = (int)min((int64_t)c->num_sms * 8, (n + 1023) / 1024);
     if (hb < 1) hb = 1;
-    radix_hist_kernel<<<hb, 256, 0, c->stream>>>(n, hash, c->hist, P);
+    switch (P) {
+    case 1: radix_hist_kernel<1><<<hb, 256, 0, c->stream>>>(n, hash, c->hist); break;
+    case 2: radix_hist_kernel<2><<<hb, 256, 0, c->stream>>>(n, hash, c->hist); break;
+    case 3: radix_hist_kernel<3><<<hb, 256, 0, c->stream>>>(n, hash, c->hist); break;
+    default: radix_hist_kernel<4><<<hb, 256, 0, c->stream>>>(n, hash, c->hist); break;
+    }
     SPH_CHECK_LAUNCH(c);
     radix_hist_scan_kernel<<<P, kRadix, 0, c->stream>>>(c->hist);
     SPH_CHECK_LAUNCH(c);
