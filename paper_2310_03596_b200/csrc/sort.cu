@@ -115,7 +115,7 @@ __global__ void __launch_bounds__(kRadix) radix_hist_scan_kernel(uint32_t *hist)
 // --------------------------------------------------------------------------- onesweep pass
 constexpr int kSortWarps = kSortThreads / 32;
 struct SortSmem {
-    uint32_t warp_hist[kSortWarps][kRadix];   // per-warp digit counts -> exclusive over the warps
+    uint16_t warp_hist[kSortWarps][kRadix];   // per-warp digit counts -> exclusive over the warps (<= 8192)
     uint32_t keys[kSortTile];
     uint32_t vals[kSortTile];
     uint32_t digit_base[kRadix];              // start of the digit's run inside the tile
@@ -135,7 +135,8 @@ onesweep_kernel(int64_t n, const uint32_t *__restrict__ keys_in, const uint32_t 
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     if (tid == 0) sm.tile = atomicAdd(ticket, 1u);
 #pragma unroll
-    for (int i = tid; i < kSortWarps * kRadix; i += kSortThreads) (&sm.warp_hist[0][0])[i] = 0;
+    for (int i = tid; i < kSortWarps * kRadix / 2; i += kSortThreads)
+        reinterpret_cast<uint32_t *>(&sm.warp_hist[0][0])[i] = 0;
     __syncthreads();
     const uint32_t tile = sm.tile;
     const int64_t tile_base = (int64_t)tile * kSortTile;
@@ -143,25 +144,17 @@ onesweep_kernel(int64_t n, const uint32_t *__restrict__ keys_in, const uint32_t 
     const int64_t chunk = tile_base + warp * (32 * kSortItems) + lane;
 
     // ---- load (warp-striped: item r of lane l = chunk[r*32 + l]) ----
-    uint32_t key[kSortItems], val[kSortItems];
+    // (values are fetched later, straight into the staging buffer: 16 fewer live registers, which
+    //  is what lets three 512-thread CTAs share an SM)
+    uint32_t key[kSortItems];
 #pragma unroll
     for (int r = 0; r < kSortItems; ++r) {
         const int64_t idx = chunk + r * 32;
         key[r] = idx < n ? __ldcs(keys_in + idx) : 0xFFFFFFFFu;
     }
-    if (!FIRST) {
-#pragma unroll
-        for (int r = 0; r < kSortItems; ++r) {
-            const int64_t idx = chunk + r * 32;
-            val[r] = idx < n ? __ldcs(vals_in + idx) : 0u;
-        }
-    } else {
-#pragma unroll
-        for (int r = 0; r < kSortItems; ++r) val[r] = (uint32_t)(chunk + r * 32);
-    }
 
     // ---- stable rank inside the warp ----
-    uint32_t rank[kSortItems];
+    uint32_t rank2[kSortItems / 2];   // two 16-bit ranks per register (rank < 512)
     const uint32_t lt = lanemask_lt();
 #pragma unroll
     for (int r = 0; r < kSortItems; ++r) {
@@ -173,11 +166,11 @@ onesweep_kernel(int64_t n, const uint32_t *__restrict__ keys_in, const uint32_t 
         // read-modify-write (shared-memory atomics with a return value measured slower)
         if (before == 0) {
             basev = sm.warp_hist[warp][d];
-            sm.warp_hist[warp][d] = basev + (uint32_t)__popc(peers);
+            sm.warp_hist[warp][d] = (uint16_t)(basev + (uint32_t)__popc(peers));
         }
         __syncwarp();
         basev = __shfl_sync(0xffffffffu, basev, __ffs(peers) - 1);
-        rank[r] = basev + before;
+        if (r & 1) rank2[r >> 1] |= (basev + before) << 16; else rank2[r >> 1] = basev + before;
     }
     __syncthreads();
 
@@ -188,7 +181,7 @@ onesweep_kernel(int64_t n, const uint32_t *__restrict__ keys_in, const uint32_t 
 #pragma unroll
         for (int w = 0; w < kSortWarps; ++w) {
             const uint32_t c = sm.warp_hist[w][d];
-            sm.warp_hist[w][d] = run;
+            sm.warp_hist[w][d] = (uint16_t)run;
             run += c;
         }
         // padding keys (0xFFFFFFFF) sit at the very end of digit 255
@@ -217,9 +210,10 @@ onesweep_kernel(int64_t n, const uint32_t *__restrict__ keys_in, const uint32_t 
 #pragma unroll
     for (int r = 0; r < kSortItems; ++r) {
         const uint32_t dg = (key[r] >> shift) & (kRadix - 1);
-        const uint32_t pos = sm.digit_base[dg] + sm.warp_hist[warp][dg] + rank[r];
+        const uint32_t pos = sm.digit_base[dg] + sm.warp_hist[warp][dg] + ((rank2[r >> 1] >> ((r & 1) * 16)) & 0xFFFFu);
         sm.keys[pos] = key[r];
-        sm.vals[pos] = val[r];
+        const int64_t idx = chunk + r * 32;
+        sm.vals[pos] = FIRST ? (uint32_t)idx : (idx < n ? __ldcs(vals_in + idx) : 0u);
     }
 
     // ---- decoupled look-back over the previous tiles ----
