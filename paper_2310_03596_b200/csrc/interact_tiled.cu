@@ -45,7 +45,7 @@ constexpr int kTW = 8;                 // warps per CTA (== kNB: warp b builds t
 constexpr int kCap = 1536;             // window records held in shared memory (64 B each)
 constexpr int kCandCap = 640;          // candidate-table entries per bucket
 constexpr int kSlots = 8;              // targets parked per warp before the epilogue
-constexpr int kAccStride = 17;         // 16 sums + 1 pad word (bank-conflict free)
+constexpr int kAccStride = 19;         // 16 sums, particle index, record index, 1 pad word (odd: conflict-free)
 constexpr int kDummy = kCap;           // kDummy + c: far-away dummy candidate of bank class c = 0..7
 static_assert(kTW == kNB, "warp b builds the candidate table of bucket b");
 static_assert((kCap + 8) * 16 < 65536 && kCap % 8 == 0, "table entries are record index * 16 in 16 bits");
@@ -477,7 +477,10 @@ interact_tiled_kernel(Packed rec, InteractIn in, const uint32_t *__restrict__ cs
                 const int idx = ((t & 4) << 1) + ((t & 2) << 1) + ((t & 1) << 1);
                 row[idx] = v[0];
                 row[idx + 1] = v[1];
-                if (t == 0) row[16] = __int_as_float(my_valid ? (int)(btb0 + my_t) : -1);
+                if (t == 0) {
+                    row[16] = __int_as_float(my_valid ? (int)(btb0 + my_t) : -1);
+                    row[17] = __int_as_float(tbase + my_t);
+                }
             }
             if (my_valid && t == 0) ++my_self;  // the self pair is not a pair (reading S15)
             ++parked;
@@ -496,8 +499,15 @@ interact_tiled_kernel(Packed rec, InteractIn in, const uint32_t *__restrict__ cs
                         for (int c = 0; c < 3; ++c) { Rr.g[c] = row[10 + c]; Rr.a[c] = row[13 + c]; }
                         float si[6];
 #pragma unroll
-                        for (int c = 0; c < 6; ++c) si[c] = in.sig[c][i];
-                        finish_particle(Rr, si, in.velr[i].w, k, out, (int64_t)i);
+                        for (int c = 0; c < 6; ++c) si[c] = 0.f;
+                        // sigma_i and rho_i come back from the target's own record in shared memory
+                        // (S = sigma / rho^2, m, V = m / rho): no global load on the epilogue's path
+                        const int rs = __float_as_int(row[17]);
+                        const float4 rb = sm.B[rs], rc = sm.C[rs], rd = sm.D[rs];
+                        const float rho = rd.z / rd.w, rho2 = rho * rho;
+                        si[0] = rc.x * rho2; si[1] = rc.w * rho2; si[2] = rb.w * rho2;
+                        si[3] = rc.y * rho2; si[4] = rd.x * rho2; si[5] = rd.y * rho2;
+                        finish_particle(Rr, si, rho, k, out, (int64_t)i);
                     }
                 }
                 __syncwarp();
@@ -519,8 +529,13 @@ interact_tiled_kernel(Packed rec, InteractIn in, const uint32_t *__restrict__ cs
                     for (int c = 0; c < 3; ++c) { Rr.g[c] = row[10 + c]; Rr.a[c] = row[13 + c]; }
                     float si[6];
 #pragma unroll
-                    for (int c = 0; c < 6; ++c) si[c] = in.sig[c][i];
-                    finish_particle(Rr, si, in.velr[i].w, k, out, (int64_t)i);
+                    for (int c = 0; c < 6; ++c) si[c] = 0.f;
+                    const int rs = __float_as_int(row[17]);
+                    const float4 rb = sm.B[rs], rc = sm.C[rs], rd = sm.D[rs];
+                    const float rho = rd.z / rd.w, rho2 = rho * rho;
+                    si[0] = rc.x * rho2; si[1] = rc.w * rho2; si[2] = rb.w * rho2;
+                    si[3] = rc.y * rho2; si[4] = rd.x * rho2; si[5] = rd.y * rho2;
+                    finish_particle(Rr, si, rho, k, out, (int64_t)i);
                 }
             }
         }
