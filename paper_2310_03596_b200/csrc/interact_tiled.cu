@@ -41,13 +41,13 @@ constexpr int kTBX = 4, kTBY = 2;      // buckets per tile along x and y
 constexpr int kNB = kTBX * kTBY;       // target buckets per tile
 constexpr int kRowsY = kTBY + 2;       // window rows along y
 constexpr int kRuns = 3 * kRowsY;      // contiguous runs of the window
-constexpr int kTW = 8;                 // warps per CTA (== kNB: warp b builds the table of bucket b)
-constexpr int kCap = 1536;             // window records held in shared memory (64 B each)
+constexpr int kTW = 12;                // warps per CTA (warp b < kNB builds the table of bucket b)
+constexpr int kCap = 1496;             // window records held in shared memory (64 B each)
 constexpr int kCandCap = 640;          // candidate-table entries per bucket
 constexpr int kSlots = 8;              // targets parked per warp before the epilogue
 constexpr int kAccStride = 19;         // 16 sums, particle index, record index, 1 pad word (odd: conflict-free)
 constexpr int kDummy = kCap;           // kDummy + c: far-away dummy candidate of bank class c = 0..7
-static_assert(kTW == kNB, "warp b builds the candidate table of bucket b");
+static_assert(kTW >= kNB, "warp b builds the candidate table of bucket b");
 static_assert((kCap + 8) * 16 < 65536 && kCap % 8 == 0, "table entries are record index * 16 in 16 bits");
 static_assert(kCandCap == 640, "three mask words cover 20 chunks of 32 table positions");
 
@@ -292,7 +292,7 @@ interact_tiled_kernel(Packed rec, InteractIn in, const uint32_t *__restrict__ cs
             }
             // shared-memory index of the first target: it sits in window run rc
             const int t_off = __shfl_sync(0xffffffffu, run_off, rc), t_lo = __shfl_sync(0xffffffffu, run_lo, rc);
-            if (lane == 0) {
+            if (lane == 0 && warp < kNB) {
                 sm.bkt_nt[warp] = nt;
                 sm.bkt_tb0[warp] = tb0;
                 sm.bkt_tsm[warp] = t_off + ((int)tb0 - t_lo);
