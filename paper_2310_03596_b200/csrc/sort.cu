@@ -159,7 +159,27 @@ onesweep_kernel(int64_t n, const uint32_t *__restrict__ keys_in, const uint32_t 
 #pragma unroll
     for (int r = 0; r < kSortItems; ++r) {
         const uint32_t d = (key[r] >> shift) & (kRadix - 1);
-        const uint32_t peers = __match_any_sync(0xffffffffu, d);
+        // MATCH.ANY costs 8 cycles per DISTINCT value and scheduler (measured: 96 cycles at 12
+        // values, 256 at 32).  The lowest digit of spatially coherent ids changes every few keys,
+        // so the first pass would pay ~12 values per round -- but there the digits of a stripe
+        // are almost always non-decreasing over the lanes, and then equal digits are adjacent:
+        // the peer group is the run between two "head" lanes (two ballots, no match).
+        uint32_t peers;
+        if (FIRST) {
+            const uint32_t dp = __shfl_up_sync(0xffffffffu, d, 1);
+            const uint32_t heads = __ballot_sync(0xffffffffu, lane == 0 || d != dp);
+            if (__ballot_sync(0xffffffffu, lane != 0 && d < dp) == 0u) {
+                const uint32_t le = lt | (1u << lane);                          // lanes <= lane
+                const uint32_t start = 31u - (uint32_t)__clz(heads & le);       // head of my run (bit 0 is set)
+                const uint32_t above = heads & ~le;                            // heads at lanes > lane
+                const uint32_t end_mask = above ? ((above & (0u - above)) - 1u) : 0xffffffffu;
+                peers = end_mask & ~((1u << start) - 1u);
+            } else {
+                peers = __match_any_sync(0xffffffffu, d);
+            }
+        } else {
+            peers = __match_any_sync(0xffffffffu, d);
+        }
         const uint32_t before = __popc(peers & lt);
         uint32_t basev = 0;
         // the histogram is private to the warp: the lowest peer books the whole group with a plain
