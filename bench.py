@@ -36,8 +36,9 @@ METRIC = "sph_step_particles_per_s"
 UNIT = "particles/s"
 FLOP_PER_CAND = 8.0      # 3 FADD + 1 FMUL + 2 FFMA
 FLOP_PER_PAIR = 66.0     # kernel factor 7 + density rate 10 + velocity gradient 22 + momentum 27
-BYTES_PER_PARTICLE = {   # algorithmic HBM bytes per particle per stage
-    "hash": 20.0, "sort": None, "reorder": 124.0, "cell_ranges": None, "comm_hash": None,
+BYTES_PER_PARTICLE = {   # algorithmic HBM bytes per particle per stage;
+                         # reorder = 124 + the 48 B of packed interaction records it writes inside sph_step
+    "hash": 20.0, "sort": None, "reorder": 172.0, "cell_ranges": None, "comm_hash": None,
     "interact": 96.0, "integrate": 156.0,
 }
 # dram__bytes_read.sum + dram__bytes_write.sum per launch of the interaction kernel from the

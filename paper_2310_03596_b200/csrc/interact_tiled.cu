@@ -556,8 +556,11 @@ int launch_interact_tiled(sph_ctx *c, int64_t n, const InteractIn &in, const uin
     rec.B = c->rec_B;
     rec.C = c->rec_C;
     rec.D = c->rec_D;
-    pack_kernel<<<div_up(n, 256), 256, 0, c->stream>>>(n, in, rec.B, rec.C, rec.D);
-    SPH_CHECK_LAUNCH(c);
+    if (!(c->rec_fresh && in.posm == reinterpret_cast<const float4 *>(c->sorted.posm))) {
+        pack_kernel<<<div_up(n, 256), 256, 0, c->stream>>>(n, in, rec.B, rec.C, rec.D);
+        SPH_CHECK_LAUNCH(c);
+    }
+    c->rec_fresh = false;
     static bool attr_set = false;
     const int smem = (int)sizeof(TileSmem);
     if (!attr_set) {

@@ -125,6 +125,7 @@ int sph_create(sph_ctx **out, const sph_params *p, int64_t max_n, void *cuda_str
     c->launches = 0;
     c->last_err = cudaSuccess;
     c->staging_ready = false;
+    c->rec_fresh = false;
     memset(&c->staging, 0, sizeof(c->staging));
 
     // grid constants: inv_edge rounded once in fp32 (reading S2)

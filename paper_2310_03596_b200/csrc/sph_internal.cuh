@@ -81,6 +81,7 @@ struct sph_ctx {
     sph_state sorted;                         // sorted copy of the state
     float4 *rec_B, *rec_C;                    // packed neighbour records of the interaction kernel
     float4 *rec_D;
+    bool rec_fresh;                           // rec_B/C/D already hold the records of `sorted` (written by reorder)
     // host-API staging (lazy)
     sph_state staging;
     bool staging_ready;
