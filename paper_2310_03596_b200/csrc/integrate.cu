@@ -1,7 +1,7 @@
 // Stage 4b: explicit integration, symplectic Euler (step g; reading S18).
-// rho += dt drho; v += dt a; sigma += dt dsig; x += dt v(new).  HBM-bound streaming kernel;
-// inside sph_step the result is scattered straight back to id order through perm, which
-// removes a separate un-permute pass.
+// rho += dt drho; v += dt a; sigma += dt dsig; x += dt v(new).  HBM-bound streaming kernel behind
+// the sph_integrate entry point.  sph_step does not launch it: there the epilogue of the
+// interaction kernel integrates and scatters to id order (interact_math.cuh, finish_particle).
 #include "sph_internal.cuh"
 
 namespace sphb {

@@ -7,16 +7,27 @@ namespace sphb {
 
 int launch_interact(sph_ctx *c, int64_t n, const sph_state *sorted, const uint32_t *sorted_hash,
                     const uint32_t *cs, const uint32_t *ce, float *drho, float *acc,
-                    float *const dsig[6], unsigned long long *pair_count)
+                    float *const dsig[6], unsigned long long *pair_count, const sph_state *fuse_out,
+                    const uint32_t *perm, float dt)
 {
     if (n == 0) return SPH_OK;
     InteractIn in;
     InteractOut out;
     in.posm = reinterpret_cast<const float4 *>(sorted->posm);
     in.velr = reinterpret_cast<const float4 *>(sorted->velr);
-    out.drho = drho;
+    out.drho = drho;   // NULL (with fuse_out set): the rates are not stored
     out.acc = reinterpret_cast<float4 *>(acc);
-    for (int i = 0; i < 6; ++i) { in.sig[i] = sorted->sig[i]; out.dsig[i] = dsig[i]; }
+    for (int i = 0; i < 6; ++i) { in.sig[i] = sorted->sig[i]; out.dsig[i] = dsig ? dsig[i] : nullptr; }
+    out.perm = nullptr;
+    out.dt = dt;
+    out.o_posm = out.o_velr = nullptr;
+    for (int i = 0; i < 6; ++i) out.o_sig[i] = nullptr;
+    if (fuse_out) {    // step g in the epilogue, scattered to id order through perm
+        out.perm = perm;
+        out.o_posm = reinterpret_cast<float4 *>(fuse_out->posm);
+        out.o_velr = reinterpret_cast<float4 *>(fuse_out->velr);
+        for (int i = 0; i < 6; ++i) out.o_sig[i] = fuse_out->sig[i];
+    }
     if (c->params.flags & SPH_FLAG_INTERACT_DIRECT)
         return launch_interact_direct(c, n, in, sorted_hash, cs, ce, out, pair_count);
     return launch_interact_tiled(c, n, in, sorted_hash, cs, ce, out, pair_count);

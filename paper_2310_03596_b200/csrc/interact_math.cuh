@@ -16,9 +16,16 @@ struct InteractIn {
     const float *sig[6];
 };
 struct InteractOut {
-    float *drho;
+    float *drho;          // rates, indexed by sorted position; all three NULL = not wanted
     float4 *acc;
     float *dsig[6];
+    // optional fused integration (step g, O9): the epilogue advances the particle and scatters
+    // it to id order through perm -- inside sph_step this removes the integrate pass (156 B per
+    // particle) and, when the caller does not ask for the rates, their 44 B store as well
+    const uint32_t *perm;  // NULL = no fused integration
+    float dt;
+    float4 *o_posm, *o_velr;
+    float *o_sig[6];
 };
 
 // MUFU.SQRT: one instruction, sqrt(0) = 0 so coincident particles need no clamp (S15)
@@ -179,9 +186,11 @@ struct PairAccum2 {
 };
 
 // Per-particle epilogue: scale by cF, add the S_i term, form the stress rate (O8) and store.
+// pos_i (x, y, z, m in the caller's coordinates) and vel_i are only read by the fused integration.
 __device__ __forceinline__ void finish_particle(const PairAccum &A, const float (&sig_i)[6],
                                                 float rho_i, const Consts &k, const InteractOut &out,
-                                                int64_t i)
+                                                int64_t i, const float4 &pos_i, float vx_i, float vy_i,
+                                                float vz_i)
 {
     const float cF = k.cF;
     const float ir = 1.0f / rho_i;
@@ -193,8 +202,11 @@ __device__ __forceinline__ void finish_particle(const PairAccum &A, const float 
     acc.y = cF * (A.a[1] + Sxy * A.g[0] + Syy * A.g[1] + Syz * A.g[2]);
     acc.z = cF * (A.a[2] + Sxz * A.g[0] + Syz * A.g[1] + Szz * A.g[2]);
     acc.w = 0.f;
-    out.drho[i] = -cF * A.dr;
-    out.acc[i] = acc;
+    const float drho = -cF * A.dr;
+    if (out.drho) {
+        out.drho[i] = drho;
+        out.acc[i] = acc;
+    }
     float L[9];
 #pragma unroll
     for (int q = 0; q < 9; ++q) L[q] = cF * A.L[q];
@@ -214,12 +226,34 @@ __device__ __forceinline__ void finish_particle(const PairAccum &A, const float 
     const float Jxy = Oxy * (syy - sxx) + Oxz * syz + Oyz * sxz;
     const float Jxz = Oxz * (szz - sxx) + Oxy * syz - Oyz * sxy;
     const float Jyz = Oyz * (szz - syy) - Oxy * sxz - Oxz * sxy;
-    out.dsig[0][i] = vol + G2 * Dxx + Jxx;
-    out.dsig[1][i] = vol + G2 * Dyy + Jyy;
-    out.dsig[2][i] = vol + G2 * Dzz + Jzz;
-    out.dsig[3][i] = G2 * Dxy + Jxy;
-    out.dsig[4][i] = G2 * Dxz + Jxz;
-    out.dsig[5][i] = G2 * Dyz + Jyz;
+    float ds[6];
+    ds[0] = vol + G2 * Dxx + Jxx;
+    ds[1] = vol + G2 * Dyy + Jyy;
+    ds[2] = vol + G2 * Dzz + Jzz;
+    ds[3] = G2 * Dxy + Jxy;
+    ds[4] = G2 * Dxz + Jxz;
+    ds[5] = G2 * Dyz + Jyz;
+    if (out.drho) {
+#pragma unroll
+        for (int c = 0; c < 6; ++c) out.dsig[c][i] = ds[c];
+    }
+    if (out.perm) {  // symplectic Euler (O9), result scattered to id order
+        const float dt = out.dt;
+        const int64_t dst = (int64_t)__ldg(out.perm + i);
+        float4 vn, pn;
+        vn.x = fmaf(dt, acc.x, vx_i);
+        vn.y = fmaf(dt, acc.y, vy_i);
+        vn.z = fmaf(dt, acc.z, vz_i);
+        vn.w = fmaf(dt, drho, rho_i);
+        pn.x = fmaf(dt, vn.x, pos_i.x);
+        pn.y = fmaf(dt, vn.y, pos_i.y);
+        pn.z = fmaf(dt, vn.z, pos_i.z);
+        pn.w = pos_i.w;
+        out.o_posm[dst] = pn;
+        out.o_velr[dst] = vn;
+#pragma unroll
+        for (int c = 0; c < 6; ++c) out.o_sig[c][dst] = fmaf(dt, ds[c], sig_i[c]);
+    }
 }
 
 // One particle of the plain global-memory walk over its 27-bucket stencil (9 contiguous runs).
@@ -266,7 +300,7 @@ __device__ __forceinline__ uint32_t direct_particle(int64_t i, int cx, int cy, i
     float si[6];
 #pragma unroll
     for (int c = 0; c < 6; ++c) si[c] = in.sig[c][i];
-    finish_particle(A, si, vi.w, k, out, i);
+    finish_particle(A, si, vi.w, k, out, i, pi, vi.x, vi.y, vi.z);
     return pairs;
 }
 

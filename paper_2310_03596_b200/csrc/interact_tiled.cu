@@ -507,7 +507,9 @@ interact_tiled_kernel(Packed rec, InteractIn in, const uint32_t *__restrict__ cs
                         const float rho = rd.z / rd.w, rho2 = rho * rho;
                         si[0] = rc.x * rho2; si[1] = rc.w * rho2; si[2] = rb.w * rho2;
                         si[3] = rc.y * rho2; si[4] = rd.x * rho2; si[5] = rd.y * rho2;
-                        finish_particle(Rr, si, rho, k, out, (int64_t)i);
+                        float4 pos_i = make_float4(0.f, 0.f, 0.f, 0.f);
+                        if (out.perm) pos_i = __ldg(in.posm + i);
+                        finish_particle(Rr, si, rho, k, out, (int64_t)i, pos_i, rb.x, rb.y, rb.z);
                     }
                 }
                 __syncwarp();
@@ -535,7 +537,9 @@ interact_tiled_kernel(Packed rec, InteractIn in, const uint32_t *__restrict__ cs
                     const float rho = rd.z / rd.w, rho2 = rho * rho;
                     si[0] = rc.x * rho2; si[1] = rc.w * rho2; si[2] = rb.w * rho2;
                     si[3] = rc.y * rho2; si[4] = rd.x * rho2; si[5] = rd.y * rho2;
-                    finish_particle(Rr, si, rho, k, out, (int64_t)i);
+                    float4 pos_i = make_float4(0.f, 0.f, 0.f, 0.f);
+                    if (out.perm) pos_i = __ldg(in.posm + i);
+                    finish_particle(Rr, si, rho, k, out, (int64_t)i, pos_i, rb.x, rb.y, rb.z);
                 }
             }
         }

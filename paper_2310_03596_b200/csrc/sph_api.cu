@@ -220,7 +220,7 @@ int sph_interact(sph_ctx *c, int64_t n, const sph_state *sorted, const uint32_t 
         if (!dsig[i]) return SPH_EINVAL;
     if (pair_count)
         SPH_CUDA_TRY(c, cudaMemsetAsync(pair_count, 0, sizeof(unsigned long long), c->stream));
-    return launch_interact(c, n, sorted, sorted_hash, cs, ce, drho, acc, dsig, pair_count);
+    return launch_interact(c, n, sorted, sorted_hash, cs, ce, drho, acc, dsig, pair_count, nullptr, nullptr, 0.f);
 }
 
 int sph_integrate(sph_ctx *c, int64_t n, float dt, const sph_state *in, const float *drho,
@@ -250,10 +250,15 @@ static int step_impl(sph_ctx *c, int64_t n, float dt, const sph_state *state, ui
     if (!boundary_ids) boundary_ids = c->s_boundary_ids;
     if (!boundary_count) boundary_count = c->s_boundary_count;
     if (!owner_counts) owner_counts = c->s_owner_counts;
-    if (!drho) drho = c->s_drho;
-    if (!acc) acc = c->s_acc;
+    // the rates are an optional product: when the caller wants none of them the fused epilogue
+    // does not store them at all
+    const bool want_rates = drho || acc || (dsig && (dsig[0] || dsig[1] || dsig[2] || dsig[3] || dsig[4] || dsig[5]));
     float *ds[6];
     for (int i = 0; i < 6; ++i) ds[i] = (dsig && dsig[i]) ? dsig[i] : c->s_dsig[i];
+    if (want_rates) {
+        if (!drho) drho = c->s_drho;
+        if (!acc) acc = c->s_acc;
+    }
 
     int rc;
     StageTimer t(c);
@@ -269,13 +274,13 @@ static int step_impl(sph_ctx *c, int64_t n, float dt, const sph_state *state, ui
                                comm_hash, boundary_ids, boundary_count, owner_counts)) != SPH_OK)
         return rc;
     t.mark();
-    if ((rc = launch_interact(c, n, &c->sorted, sorted_hash, cell_start, cell_end, drho, acc, ds,  // e, f
-                              pair_count)) != SPH_OK)
+    // steps e, f and g: the interaction epilogue integrates (O9) and scatters the result back to
+    // id order through perm; `state` is only written, the loops read the sorted copy
+    if ((rc = launch_interact(c, n, &c->sorted, sorted_hash, cell_start, cell_end, want_rates ? drho : nullptr,
+                              want_rates ? acc : nullptr, want_rates ? ds : nullptr, pair_count, state, perm,
+                              dt)) != SPH_OK)
         return rc;
     t.mark();
-    const float *cds[6] = {ds[0], ds[1], ds[2], ds[3], ds[4], ds[5]};
-    if ((rc = launch_integrate(c, n, dt, &c->sorted, drho, acc, cds, state, perm)) != SPH_OK)    // step g
-        return rc;
     t.mark();
     return SPH_OK;
 }
