@@ -389,13 +389,13 @@ interact_tiled_kernel(Packed rec, InteractIn in, const uint32_t *__restrict__ cs
                 test_push2(m2, pa, ax23, ay23, az23, nt23);
                 test_push2(m2, pa, ax01, ay01, az01, nt01);
             }
-#pragma unroll 2
+#pragma unroll 4
             for (int s = min(nch, 16) - 1; s >= 8; --s) {
                 const float4 pa = ld_rec(sm.A, cb[32 * s]);
                 test_push2(m1, pa, ax23, ay23, az23, nt23);
                 test_push2(m1, pa, ax01, ay01, az01, nt01);
             }
-#pragma unroll 2
+#pragma unroll 4
             for (int s = min(nch, 8) - 1; s >= 0; --s) {
                 const float4 pa = ld_rec(sm.A, cb[32 * s]);
                 test_push2(m0, pa, ax23, ay23, az23, nt23);
