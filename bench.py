@@ -43,7 +43,7 @@ BYTES_PER_PARTICLE = {   # algorithmic HBM bytes per particle per stage (DESIGN.
 }
 # dram__bytes_read.sum + dram__bytes_write.sum per launch of the interaction kernel from the
 # committed `ncu --set full` capture (profiles/), keyed by config; None until captured.
-NCU_TRAFFIC_BYTES = {1: 130.04e6}   # profiles/r01c_interact_v6_ncu_full.md (104.6 MB read + 25.4 MB written)
+NCU_TRAFFIC_BYTES = {1: 93.69e6}   # profiles/r01d_interact_v6_ncu_full.md (68.6 MB read + 25.1 MB written)
 
 
 def load_peaks():
