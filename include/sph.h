@@ -139,7 +139,13 @@ int sph_integrate(sph_ctx *ctx, int64_t n, float dt, const sph_state *in, const 
  * integrate.  `state` is in ID ORDER on entry and on exit (so the (hash, id) tie-break stays
  * exact when every step re-sorts, reading S5).  Every output pointer below is optional (NULL =
  * keep it in ctx scratch); when given it receives exactly what the stage call of the same name
- * would produce (rates indexed by sorted position). */
+ * would produce (rates indexed by sorted position).  Two stage boundaries are fused inside this
+ * call: the reorder pass also writes the interaction kernel's packed records, and the
+ * interaction epilogue integrates and scatters to id order.  The rates drho / acc / dsig are
+ * intermediates of that epilogue: if all three are NULL they are not stored anywhere; if any is
+ * given all of them are computed as usual (missing ones go to ctx scratch).  The integrated
+ * state agrees with sph_integrate of the same rates to 3 ulp (sigma and rho re-enter the
+ * epilogue as sigma / rho^2 * rho^2 and m / (m / rho)). */
 int sph_step(sph_ctx *ctx, int64_t n, float dt, const sph_state *state,
              uint32_t *hash, uint32_t *sorted_hash, uint32_t *perm,
              uint32_t *cell_start, uint32_t *cell_end, uint32_t *comm_hash,
