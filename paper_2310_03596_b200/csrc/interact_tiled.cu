@@ -8,11 +8,12 @@
 //    3 (kTBY + 2) rows of kTBX + 2 buckets around it, i.e. 12 contiguous runs of the sorted arrays.
 //    The window's packed records, four 16-byte parts per particle (A = x,y,z,m -> after the shift
 //    x',y',z',|p'|^2; B = vx,vy,vz,Szz; C = Sxx,Sxy,Sxy,Syy; D = Sxz,Syz,m,V with V = m/rho,
-//    S = sigma/rho^2; B, C, D written by pack_kernel in the pair layout of PairAccum2) are brought
+//    S = sigma/rho^2; B, C, D written by the reorder pass inside sph_step, else by pack_kernel, in
+//    the pair layout of PairAccum2) are brought
 //    to shared memory with 1-D TMA bulk copies (cp.async.bulk + mbarrier), no register staging.
 //  * Warp b builds the candidate table of bucket b once: the 27-bucket stencil as shared-memory
 //    record offsets, every run padded so that (table position) == (record index) mod 8.
-//  * Work unit = 4 consecutive targets of one bucket, dealt round-robin to the 8 warps.
+//  * Work unit = 4 consecutive targets of one bucket, dealt round-robin to the 12 warps.
 //    Phase 1 (distance tests): lane l tests candidate 32 s + l of the table against the 4 targets
 //    held in registers as two fp32 pairs (one 128-bit shared load per 128 tests; expanded-form
 //    test in tile-local coordinates, 4 FFMA2 per 2 tests) and records the outcome as one bit per
@@ -27,7 +28,8 @@
 //    max-over-lanes rounds; idle lanes evaluate the dummy record of their class), paid on a pair
 //    body that is packed (PairAccum2: FFMA2 / FMUL2 / FADD2, 30 issue slots per pair instead
 //    of 46).  The 16 partial sums are reduced over the 8 lanes, parked in shared memory, and a
-//    lane-per-target epilogue forms the rates (O8) and stores them.
+//    lane-per-target epilogue forms the rates (O8), stores them if asked to, and -- inside
+//    sph_step -- integrates the particle (O9) and scatters it to id order through perm.
 //  * No pair is skipped or evaluated twice: the self pair is accepted like any other (it
 //    contributes exactly zero because x_ii = 0) and is subtracted from pair_count.
 // Tiles whose window does not fit the shared-memory budget and buckets whose table overflows
