@@ -119,14 +119,16 @@ def _fullsize_case(sph, oracle, k, steps_before, expect_boundary):
 
 def test_config1_full_size(sph, oracle):
     """configs[1], 1 M particles, the workload bench.py times by default: the oracle's integer
-    stages in full (bit-exact) and 3 000 sampled particles for the floats, at step 3."""
-    errs = _fullsize_case(sph, oracle, 1, steps_before=2, expect_boundary=(0.15, 0.27))
+    stages in full (bit-exact) and 3 000 sampled particles for the floats, at the LAST of the
+    config's 10 steps (re-hash and re-sort every step)."""
+    errs = _fullsize_case(sph, oracle, 1, steps_before=9, expect_boundary=(0.15, 0.27))
     assert max(errs.values()) <= parity.RATE_TOL
 
 
 def test_config2_full_size(sph, oracle):
-    """configs[2], 8 M particles, volumetric exchange region (everything is a boundary particle)."""
-    _fullsize_case(sph, oracle, 2, steps_before=1, expect_boundary=(0.999, 1.0))
+    """configs[2], 8 M particles, volumetric exchange region (everything is a boundary particle);
+    checked at the last of its 10 steps."""
+    _fullsize_case(sph, oracle, 2, steps_before=9, expect_boundary=(0.999, 1.0))
 
 
 @pytest.mark.skipif(os.environ.get("SPH_SKIP_64M") == "1", reason="SPH_SKIP_64M=1")
