@@ -37,6 +37,8 @@ def _load():
     lib.orc_comm_hash.restype = None
     lib.orc_boundary.argtypes = [i64, vp, vp, vp, C.c_int32, vp, vp]
     lib.orc_boundary.restype = i64
+    lib.orc_pack_boundary.argtypes = [i64, i64, vp, vp, C.c_int32] + [vp] * 9
+    lib.orc_pack_boundary.restype = None
     lib.orc_kernel_W.argtypes = [f64, f64]
     lib.orc_kernel_W.restype = f64
     lib.orc_kernel_F.argtypes = [f64, f64]
@@ -119,6 +121,37 @@ def boundary(comm_hash_, perm, sorted_owner, n_owners: int):
     if m < 0:
         raise MemoryError("orc_boundary")
     return ids[:m].copy(), counts
+
+
+@dataclass
+class PackedBoundary:
+    offsets: np.ndarray      # [n_owners + 1] u32, segment g = [offsets[g], offsets[g + 1])
+    ids: np.ndarray          # [M] u32, per segment in (hash, id) order
+    posm: np.ndarray         # [M,4] f32
+    velr: np.ndarray         # [M,4] f32
+    sig: np.ndarray          # [6,M] f32
+    owner: np.ndarray        # [M] i32
+
+
+def pack_boundary(boundary_ids, owner, n_owners: int, posm, velr, sig) -> PackedBoundary:
+    """Per-owner send buffers (sph_oracle.c O5b).  State arrays in id order; sig is [6, n]."""
+    boundary_ids = _c(boundary_ids, np.uint32)
+    owner = _c(owner, np.int32)
+    posm = _c(posm, np.float32)
+    velr = _c(velr, np.float32)
+    sig = _c(sig, np.float32)
+    n, m = posm.shape[0], boundary_ids.shape[0]
+    off = np.zeros(n_owners + 1, np.uint32)
+    ids = np.empty(max(m, 1), np.uint32)
+    pp = np.empty((max(m, 1), 4), np.float32)
+    pv = np.empty((max(m, 1), 4), np.float32)
+    ps = np.empty((6, max(m, 1)), np.float32)
+    po = np.empty(max(m, 1), np.int32)
+    if m == 0:
+        return PackedBoundary(off, ids[:0], pp[:0], pv[:0], ps[:, :0], po[:0])
+    _load().orc_pack_boundary(n, m, _p(boundary_ids), _p(owner), int(n_owners), _p(posm), _p(velr),
+                              _p(sig), _p(off), _p(ids), _p(pp), _p(pv), _p(ps), _p(po))
+    return PackedBoundary(off, ids, pp, pv, ps, po)
 
 
 @dataclass

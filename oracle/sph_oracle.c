@@ -20,7 +20,8 @@
  * enumeration, kernel normalisation integral and dW/dr by finite differences, exact momentum
  * conservation, zero rates for uniform translation, continuum limits of the gradient operators
  * (sign and index conventions), Hooke / Jaumann textbook cases, expm() finite rotation,
- * cell-table identities, sort vs numpy.lexsort, hash at bucket faces.  No function is unpinned.
+ * cell-table identities, sort vs numpy.lexsort, hash at bucket faces, per-owner send buffers vs a
+ * stable numpy argsort.  No function is unpinned.
  */
 #include <math.h>
 #include <stdint.h>
@@ -167,6 +168,40 @@ int64_t orc_boundary(int64_t n, const uint32_t *comm_hash, const uint32_t *perm,
     free(p);
     free(owner_of_id);
     return m;
+}
+
+/* ------------------------------------------------------------------------------------------
+ * O5b  Per-owner send buffers ("each GPU ... the data that
+ * shall be broadcasted to the other GPUs can be isolated", PAPER.md:23 step d "Each GPU
+ * broadcasts its MGPU boundary particle data").  In the paper every GPU isolates ITS OWN boundary
+ * particles; with owner labels that is the boundary list cut into one segment per owner.
+ * Definition written out: segment g = the entries of the boundary list (already in (hash, id)
+ * order) whose owner is g, in list order; offsets[g] = number of entries in segments < g,
+ * offsets[n_owners] = M; the packed records are the id-ordered state read at packed_ids.
+ * posm / velr are [n][4], sig is [6][n] (SoA); packed sig is [6][M].
+ * ---------------------------------------------------------------------------------------- */
+void orc_pack_boundary(int64_t n, int64_t m, const uint32_t *boundary_ids, const int32_t *owner,
+                       int32_t n_owners, const float *posm, const float *velr, const float *sig,
+                       uint32_t *offsets, uint32_t *packed_ids, float *p_posm, float *p_velr,
+                       float *p_sig, int32_t *p_owner)
+{
+    int64_t j = 0;
+    for (int32_t g = 0; g < n_owners; ++g) {
+        offsets[g] = (uint32_t)j;
+        for (int64_t k = 0; k < m; ++k) {
+            const uint32_t id = boundary_ids[k];
+            if (owner[id] != g) continue;
+            packed_ids[j] = id;
+            for (int a = 0; a < 4; ++a) {
+                p_posm[4 * j + a] = posm[4 * (int64_t)id + a];
+                p_velr[4 * j + a] = velr[4 * (int64_t)id + a];
+            }
+            for (int c = 0; c < 6; ++c) p_sig[(int64_t)c * m + j] = sig[(int64_t)c * n + id];
+            p_owner[j] = owner[id];
+            ++j;
+        }
+    }
+    offsets[n_owners] = (uint32_t)j;
 }
 
 /* ------------------------------------------------------------------------------------------

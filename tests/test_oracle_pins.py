@@ -455,3 +455,40 @@ def test_expected_boundary_fractions():
     w = W.config(2, side=32)
     r, *_ = sorted_view(w)
     assert r.boundary_ids.size == w.n
+
+
+# ----------------------------------------------------------------------------- NEXT-1: send buffers
+@pytest.mark.parametrize("make", [lambda: W.config(0), lambda: W.config(2, side=20),
+                                  lambda: W.config(3, scale=0.05)])
+def test_pack_boundary_vs_stable_argsort_and_invariants(make):
+    """Per-owner send buffers (O5b) against the library statement of the same
+    thing -- a STABLE argsort of the boundary list on the owner label -- and the invariants that
+    define it: segments partition the boundary set, each is a subsequence of the (hash, id)
+    ordered list, sizes equal owner_counts, records are the state at the packed ids."""
+    w = make()
+    r = orc.step(w.posm, w.velr, w.sig, w.owner, w.origin, w.dims, w.h, w.K, w.G, w.n_owners, w.dt,
+                 floats=False)
+    pb = orc.pack_boundary(r.boundary_ids, w.owner, w.n_owners, w.posm, w.velr, w.sig)
+    ids = r.boundary_ids
+    order = np.argsort(w.owner[ids], kind="stable")
+    np.testing.assert_array_equal(pb.ids, ids[order])
+    np.testing.assert_array_equal(np.diff(pb.offsets.astype(np.int64)), r.owner_counts)
+    assert pb.offsets[0] == 0 and pb.offsets[-1] == ids.size
+    assert sorted(pb.ids.tolist()) == sorted(ids.tolist())
+    pos_in_list = np.empty(w.n, np.int64); pos_in_list[ids] = np.arange(ids.size)
+    for g in range(w.n_owners):
+        seg = pb.ids[pb.offsets[g]:pb.offsets[g + 1]]
+        assert (w.owner[seg] == g).all()
+        assert (np.diff(pos_in_list[seg]) > 0).all()        # list order kept inside a segment
+    np.testing.assert_array_equal(pb.posm, w.posm[pb.ids])
+    np.testing.assert_array_equal(pb.velr, w.velr[pb.ids])
+    np.testing.assert_array_equal(pb.sig, w.sig[:, pb.ids])
+    np.testing.assert_array_equal(pb.owner, w.owner[pb.ids])
+
+
+def test_pack_boundary_single_owner_is_empty():
+    w = W.lattice_block(8, 8, 8, 0.1, 3, owners=("single",))
+    r = orc.step(w.posm, w.velr, w.sig, w.owner, w.origin, w.dims, w.h, w.K, w.G, w.n_owners, w.dt,
+                 floats=False)
+    pb = orc.pack_boundary(r.boundary_ids, w.owner, w.n_owners, w.posm, w.velr, w.sig)
+    assert pb.ids.size == 0 and (pb.offsets == 0).all()
