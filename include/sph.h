@@ -152,6 +152,23 @@ int sph_step(sph_ctx *ctx, int64_t n, float dt, const sph_state *state,
              uint32_t *boundary_ids, uint32_t *boundary_count, uint32_t *owner_counts,
              float *drho, float *acc, float *const dsig[6], unsigned long long *pair_count);
 
+/* NEXT-1 -- per-owner send buffers: the product of step d ("the data
+ * that shall be broadcasted to the other GPUs can be isolated"; "Each GPU broadcasts
+ * its MGPU boundary particle data").  In the paper every GPU isolates its OWN boundary particles;
+ * with owner labels that is the boundary list cut into one segment per owner:
+ *   segment g = the entries of boundary_ids (already in (hash, id) order) whose owner is g, in
+ *   list order;  owner_offsets[g] = size of the segments before g, owner_offsets[n_owners] = m;
+ *   packed_ids = the segments back to back;  packed->X[j] = state->X[packed_ids[j]] for posm,
+ *   velr, sig[0..5], owner -- contiguous per owner, ready to be handed to a collective.
+ * m = number of boundary particles, a HOST value (read boundary_count after synchronising the
+ * stream: the exchange needs the size on the host anyway); 0 <= m <= n.
+ * In: state dev, id order, length n; boundary_ids dev [m].
+ * Out: owner_offsets dev [n_owners + 1]; packed_ids dev [m]; packed dev arrays of capacity m
+ * (packed->sig[c] are six separate planes).  Not part of sph_step. */
+int sph_pack_boundary(sph_ctx *ctx, int64_t n, int64_t m, const sph_state *state,
+                      const uint32_t *boundary_ids, uint32_t *owner_offsets, uint32_t *packed_ids,
+                      const sph_state *packed);
+
 /* End-to-end variant with HOST buffers (pinned memory recommended): uploads the id-ordered state,
  * runs `steps` iterations, downloads the state, the boundary list of the last step and the
  * counters, and synchronises the stream before returning.  Device staging lives in the ctx

@@ -346,6 +346,56 @@ int launch_sort(sph_ctx *c, int64_t n, const uint32_t *hash, uint32_t *sorted_ha
     return SPH_OK;
 }
 
+// --------------------------------------------------------------------------- stable partition
+// NEXT-1 (per-owner send buffers): cut the boundary list into one segment per owner.  A stable
+// partition on a label < 256 is exactly ONE onesweep pass (digit = the label) with the list
+// entries as values; the exclusive digit histogram is the table of segment offsets.
+__global__ void __launch_bounds__(256)
+gather_label_kernel(int64_t m, const uint32_t *__restrict__ ids, const int32_t *__restrict__ label,
+                    uint32_t *__restrict__ key)
+{
+    const int64_t k = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (k < m) key[k] = (uint32_t)__ldg(label + __ldcs(ids + k)) & (kRadix - 1);
+}
+
+__global__ void segment_offsets_kernel(const uint32_t *__restrict__ hist_excl, int n_labels, uint32_t m,
+                                       uint32_t *__restrict__ offsets)
+{
+    const int g = threadIdx.x;
+    if (g < n_labels) offsets[g] = hist_excl[g];
+    if (g == n_labels) offsets[g] = m;
+}
+
+int launch_partition_by_label(sph_ctx *c, int64_t m, const uint32_t *ids, const int32_t *label, int n_labels,
+                              uint32_t *offsets, uint32_t *ids_out)
+{
+    if (m == 0) {
+        SPH_CUDA_TRY(c, cudaMemsetAsync(offsets, 0, sizeof(uint32_t) * (n_labels + 1), c->stream));
+        return SPH_OK;
+    }
+    uint32_t *key = c->alt_keys, *key_out = c->alt_vals;      // scratch of the sort (stream-ordered)
+    const int64_t tiles = (m + kSortTile - 1) / kSortTile;
+    SPH_CUDA_TRY(c, cudaMemsetAsync(c->hist, 0, sizeof(uint32_t) * kRadix, c->stream));
+    SPH_CUDA_TRY(c, cudaMemsetAsync(c->tile_counter, 0, sizeof(uint32_t), c->stream));
+    SPH_CUDA_TRY(c, cudaMemsetAsync(c->tile_status, 0, sizeof(uint32_t) * (size_t)tiles * kRadix, c->stream));
+    gather_label_kernel<<<div_up(m, 256), 256, 0, c->stream>>>(m, ids, label, key);
+    SPH_CHECK_LAUNCH(c);
+    int hb = (int)min((int64_t)c->num_sms * 8, (m + 1023) / 1024);
+    if (hb < 1) hb = 1;
+    radix_hist_kernel<1><<<hb, 256, 0, c->stream>>>(m, key, c->hist);
+    SPH_CHECK_LAUNCH(c);
+    radix_hist_scan_kernel<<<1, kRadix, 0, c->stream>>>(c->hist);
+    SPH_CHECK_LAUNCH(c);
+    segment_offsets_kernel<<<1, 64, 0, c->stream>>>(c->hist, n_labels, (uint32_t)m, offsets);
+    SPH_CHECK_LAUNCH(c);
+    SPH_CUDA_TRY(c, cudaFuncSetAttribute(onesweep_kernel<false>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                         (int)sizeof(SortSmem)));
+    onesweep_kernel<false><<<(unsigned)tiles, kSortThreads, sizeof(SortSmem), c->stream>>>(
+        m, key, ids, key_out, ids_out, c->hist, c->tile_status, c->tile_counter, 0);
+    SPH_CHECK_LAUNCH(c);
+    return SPH_OK;
+}
+
 // --------------------------------------------------------------------------- generic scan
 // Single-pass exclusive prefix sum of uint32 with decoupled look-back (used for the compaction
 // offsets of the boundary-particle list).  Totals must stay below 2^30.

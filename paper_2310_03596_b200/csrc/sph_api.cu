@@ -193,6 +193,17 @@ int sph_reorder(sph_ctx *c, int64_t n, const uint32_t *perm, const sph_state *in
     return launch_reorder(c, n, perm, in, out);
 }
 
+int sph_pack_boundary(sph_ctx *c, int64_t n, int64_t m, const sph_state *state, const uint32_t *boundary_ids,
+                      uint32_t *owner_offsets, uint32_t *packed_ids, const sph_state *packed)
+{
+    if (!n_ok(c, n) || m < 0 || m > n || !state_ok(state) || !owner_offsets) return SPH_EINVAL;
+    if (m > 0 && (!boundary_ids || !packed_ids || !state_ok(packed))) return SPH_EINVAL;
+    int rc = launch_partition_by_label(c, m, boundary_ids, state->owner, c->params.n_owners, owner_offsets,
+                                       packed_ids);
+    if (rc != SPH_OK || m == 0) return rc;
+    return launch_reorder(c, m, packed_ids, state, packed);   // gather the records segment by segment
+}
+
 int sph_cell_ranges(sph_ctx *c, int64_t n, const uint32_t *sorted_hash, uint32_t *cs, uint32_t *ce)
 {
     if (!n_ok(c, n) || !sorted_hash || !cs || !ce) return SPH_EINVAL;

@@ -123,6 +123,8 @@ int launch_interact(sph_ctx *c, int64_t n, const sph_state *sorted, const uint32
 int launch_integrate(sph_ctx *c, int64_t n, float dt, const sph_state *in, const float *drho,
                      const float *acc, const float *const dsig[6], const sph_state *out,
                      const uint32_t *scatter_perm /* NULL = elementwise */);
+int launch_partition_by_label(sph_ctx *c, int64_t m, const uint32_t *ids, const int32_t *label, int n_labels,
+                              uint32_t *offsets, uint32_t *ids_out);
 int launch_scan_exclusive(sph_ctx *c, int64_t n, const uint32_t *in, uint32_t *out,
                           uint32_t *total /* dev scalar */);
 

@@ -28,7 +28,7 @@ FLAG_INTERACT_DIRECT = 1
 
 EXPORTS = (
     "sph_create", "sph_destroy", "sph_hash", "sph_sort", "sph_reorder", "sph_cell_ranges",
-    "sph_comm_hash", "sph_interact", "sph_integrate", "sph_step", "sph_step_host",
+    "sph_comm_hash", "sph_interact", "sph_integrate", "sph_step", "sph_step_host", "sph_pack_boundary",
     "sph_enable_timing", "sph_get_timing", "sph_launch_count", "sph_strerror",
     "sph_last_cuda_error",
 )
@@ -73,6 +73,7 @@ def load_library() -> C.CDLL:
     lib.sph_integrate.argtypes = [vp, i64, f32, sp, vp, vp, C.POINTER(vp * 6), sp]
     lib.sph_step.argtypes = [vp, i64, f32, sp] + [vp] * 11 + [C.POINTER(vp * 6), vp]
     lib.sph_step_host.argtypes = [vp, i64, f32, i32, sp, vp, vp, vp]
+    lib.sph_pack_boundary.argtypes = [vp, i64, i64, sp, vp, vp, vp, sp]
     lib.sph_enable_timing.argtypes = [vp, i32]
     lib.sph_get_timing.argtypes = [vp, C.POINTER(f32 * 8)]
     lib.sph_launch_count.argtypes = [vp]
@@ -332,6 +333,18 @@ class Context:
         self._chk(rc, "sph_step")
         return out
 
+    def sph_pack_boundary(self, state: State, boundary_ids: torch.Tensor, m: int):
+        """Per-owner send buffers (NEXT-1): returns (owner_offsets [n_owners + 1], packed_ids [m],
+        packed State of length m).  m is the host value of boundary_count."""
+        m = int(m)
+        offs = self._i32(self.n_owners + 1)
+        ids = self._i32(max(m, 1))
+        packed = State.empty(max(m, 1), self.device)
+        a, b = state._c(), packed._c()
+        self._chk(self.lib.sph_pack_boundary(self.handle, state.n, m, C.byref(a), boundary_ids.data_ptr(),
+                                             offs.data_ptr(), ids.data_ptr(), C.byref(b)), "sph_pack_boundary")
+        return offs, ids[:m], State(packed.posm[:m], packed.velr[:m], packed.sig[:, :m], packed.owner[:m])
+
     def sph_step_host(self, host_state: State, dt, steps=1, boundary_ids: np.ndarray | None = None):
         """End to end with HOST buffers (pinned recommended): H2D, `steps` iterations, D2H, sync.
         Returns (boundary_count, pair_count) as Python ints; host_state is updated in place."""
@@ -356,3 +369,4 @@ def sph_interact(ctx, *a, **k): return ctx.sph_interact(*a, **k)
 def sph_integrate(ctx, *a, **k): return ctx.sph_integrate(*a, **k)
 def sph_step(ctx, *a, **k): return ctx.sph_step(*a, **k)
 def sph_step_host(ctx, *a, **k): return ctx.sph_step_host(*a, **k)
+def sph_pack_boundary(ctx, *a, **k): return ctx.sph_pack_boundary(*a, **k)

@@ -231,3 +231,33 @@ def test_repeated_runs_are_bit_identical(sph):
             for a, b in zip(ref, got):
                 assert torch.equal(a, b)
     ctx.close()
+
+
+# ------------------------------------------------------------------ NEXT-1: per-owner send buffers
+@pytest.mark.parametrize("make", [lambda: wl.config(0), lambda: wl.config(1, side=33),
+                                  lambda: wl.config(2, side=37), lambda: wl.config(3, scale=0.1),
+                                  lambda: wl.lattice_block(12, 12, 12, 0.1, 5, owners=("single",))],
+                         ids=["cfg0", "cfg1", "cfg2", "cfg3", "one-owner"])
+def test_pack_boundary_matches_oracle(sph, oracle, make):
+    """sph_pack_boundary against oracle.pack_boundary: pure index and copy work,
+    so everything is bit-exact.  The boundary list fed to both sides is the GPU step's, which the
+    lock-step tests above pin to the oracle's."""
+    w = make()
+    ctx = sph.Context.for_workload(w)
+    state = sph.State.from_numpy(w.posm, w.velr, w.sig, w.owner)
+    out = ctx.alloc_outputs(w.n)
+    ctx.sph_step(state, w.dt, out)
+    torch.cuda.synchronize()
+    m = int(parity.u32(out.boundary_count)[0])
+    offs, ids, packed = ctx.sph_pack_boundary(state, out.boundary_ids, m)
+    torch.cuda.synchronize()
+    ref = oracle.pack_boundary(parity.u32(out.boundary_ids)[:m], state.owner.cpu().numpy(), w.n_owners,
+                               state.posm.cpu().numpy(), state.velr.cpu().numpy(), state.sig.cpu().numpy())
+    np.testing.assert_array_equal(parity.u32(offs), ref.offsets)
+    np.testing.assert_array_equal(parity.u32(ids), ref.ids)
+    np.testing.assert_array_equal(packed.posm.cpu().numpy(), ref.posm)
+    np.testing.assert_array_equal(packed.velr.cpu().numpy(), ref.velr)
+    np.testing.assert_array_equal(packed.sig.cpu().numpy(), ref.sig)
+    np.testing.assert_array_equal(packed.owner.cpu().numpy(), ref.owner)
+    np.testing.assert_array_equal(np.diff(ref.offsets.astype(np.int64)), parity.u32(out.owner_counts))
+    ctx.close()
