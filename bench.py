@@ -248,7 +248,29 @@ def run_ours(args, rank, world, local_rank):
         stage_ms = ctx.get_timing()
     total_ms = max_over_ranks(total_ms, world, dev)
 
-    # ---- end to end through the C-ABI with pinned host buffers ----
+    # ---- NEXT-1 (not part of the step metric): per-owner send buffers of the last boundary list ----
+    pack = None
+    if boundary > 0:
+        bids_dev = torch.empty(n, dtype=torch.int32, device=dev)
+        bcnt = torch.zeros(1, dtype=torch.int32, device=dev)
+        o2 = ctx.alloc_outputs(n)
+        ctx.sph_step(state.clone(), w.dt, o2)
+        torch.cuda.synchronize(dev)
+        m_b = int(sph.as_u32(o2.boundary_count)[0])
+        pk_ms = []
+        for _ in range(5):
+            flush.zero_()
+            a_, b_ = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            a_.record()
+            ctx.sph_pack_boundary(state, o2.boundary_ids, m_b)
+            b_.record()
+            torch.cuda.synchronize(dev)
+            pk_ms.append(a_.elapsed_time(b_))
+        pk = float(np.median(pk_ms[1:]))
+        pack = {"ms": round(pk, 4), "boundary_particles": m_b, "bytes_per_boundary_particle": 156,
+                "note": "includes the allocation of the output tensors by the binding"}
+        del o2, bids_dev, bcnt
+
     host = sph.State.from_numpy(w.posm, w.velr, w.sig, w.owner, device="cpu", pin=True)
     bids = torch.empty(n, dtype=torch.int32).pin_memory().numpy().view(np.uint32)
     ctx.sph_step_host(host, w.dt, 1, bids)               # warm-up (allocates staging)
@@ -314,6 +336,10 @@ def run_ours(args, rank, world, local_rank):
                      "interact_hbm_gbs": BYTES_PER_PARTICLE["interact"] * n / t_int / 1e9},
         "stages": stages,
     }
+    if pack:
+        pack["gbs"] = round(pack["bytes_per_boundary_particle"] * pack["boundary_particles"] / (pack["ms"] * 1e-3) / 1e9, 1)
+        pack["hbm_frac"] = round(pack["gbs"] / peaks["hbm_gbs"], 3)
+        line["next1_pack_boundary"] = pack
     if world == 1 and not args.no_cpu_baseline:
         cb = time_oracle(w, args.cpu_sample, 3, 1)
         line["cpu_baseline"] = {k_: cb[k_] for k_ in ("value", "unit", "cores", "kind", "sample")}

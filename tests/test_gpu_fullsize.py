@@ -111,6 +111,16 @@ def _fullsize_case(sph, oracle, k, steps_before, expect_boundary):
                        ("rho", g_vel[:, 3], vo[:, 3]), ("sig", g_sig, so)):
         e = parity.field_err(g, r)
         assert e <= parity.STATE_TOL, (name, e)
+    # NEXT-1: per-owner send buffers of this step's boundary list, from the integrated state
+    offs, pids, packed = ctx.sph_pack_boundary(state, out.boundary_ids, m)
+    torch.cuda.synchronize()
+    ref = oracle.pack_boundary(parity.u32(out.boundary_ids)[:m], owner, w.n_owners, state.posm.cpu().numpy(),
+                               state.velr.cpu().numpy(), state.sig.cpu().numpy())
+    np.testing.assert_array_equal(parity.u32(offs), ref.offsets)
+    np.testing.assert_array_equal(parity.u32(pids), ref.ids)
+    np.testing.assert_array_equal(packed.posm.cpu().numpy(), ref.posm)
+    np.testing.assert_array_equal(packed.sig.cpu().numpy(), ref.sig)
+    del packed, ref
     # untouched particles elsewhere keep mass and owner
     np.testing.assert_array_equal(state.owner.cpu().numpy(), owner)
     ctx.close()
