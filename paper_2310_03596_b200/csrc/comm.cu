@@ -56,14 +56,22 @@ owner_mask_kernel(int64_t n, const uint32_t *__restrict__ sorted_hash,
     if (cur != 0xFFFFFFFFu) atomicOr(cell_mask + cur, m);
 }
 
+// One thread per 4 consecutive buckets of a grid row: the 9 stencil rows are read once as 6 masks
+// each (54 loads for 4 buckets instead of 108) and OR-ed with a sliding window.
+constexpr int kFlagCells = 4;
+
 __global__ void __launch_bounds__(256)
 stencil_flag_kernel(Grid g, const uint32_t *__restrict__ cell_mask, const uint32_t *__restrict__ cs,
                     const uint32_t *__restrict__ ce, uint32_t *__restrict__ flag_count)
 {
-    const uint32_t c = blockIdx.x * blockDim.x + threadIdx.x;
-    if (c >= g.n_cells) return;
-    const int cx = c % g.nx, cy = (c / g.nx) % g.ny, cz = c / (g.nx * g.ny);
-    uint32_t m = 0;
+    const int groups_x = (g.nx + kFlagCells - 1) / kFlagCells;
+    const int64_t t = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (t >= (int64_t)groups_x * g.ny * g.nz) return;
+    const int gx = (int)(t % groups_x), cy = (int)((t / groups_x) % g.ny), cz = (int)(t / ((int64_t)groups_x * g.ny));
+    const int x0 = gx * kFlagCells;
+    uint32_t col[kFlagCells + 2];   // OR over the 9 rows of the masks at x0 - 1 .. x0 + kFlagCells
+#pragma unroll
+    for (int i = 0; i < kFlagCells + 2; ++i) col[i] = 0u;
 #pragma unroll
     for (int dz = -1; dz <= 1; ++dz) {
         const int z = cz + dz;
@@ -74,15 +82,22 @@ stencil_flag_kernel(Grid g, const uint32_t *__restrict__ cell_mask, const uint32
             if (y < 0 || y >= g.ny) continue;
             const uint32_t row = (uint32_t)g.nx * ((uint32_t)y + (uint32_t)g.ny * (uint32_t)z);
 #pragma unroll
-            for (int dx = -1; dx <= 1; ++dx) {
-                const int x = cx + dx;
-                if (x < 0 || x >= g.nx) continue;
-                m |= __ldg(cell_mask + row + x);
+            for (int i = 0; i < kFlagCells + 2; ++i) {
+                const int x = x0 - 1 + i;
+                if (x >= 0 && x < g.nx) col[i] |= __ldg(cell_mask + row + x);
             }
         }
     }
-    // an empty bucket contributes no particles whatever its stencil holds
-    flag_count[c] = (__popc(m) >= 2) ? (ce[c] - cs[c]) : 0u;
+    const uint32_t row0 = (uint32_t)g.nx * ((uint32_t)cy + (uint32_t)g.ny * (uint32_t)cz);
+#pragma unroll
+    for (int i = 0; i < kFlagCells; ++i) {
+        const int x = x0 + i;
+        if (x >= g.nx) break;
+        const uint32_t m = col[i] | col[i + 1] | col[i + 2];
+        const uint32_t c = row0 + (uint32_t)x;
+        // an empty bucket contributes no particles whatever its stencil holds
+        flag_count[c] = (__popc(m) >= 2) ? (ce[c] - cs[c]) : 0u;
+    }
 }
 
 constexpr int kCompItems = 8;  // sorted particles per thread (two 128-bit loads per array in flight)
@@ -208,8 +223,11 @@ int launch_comm_hash(sph_ctx *c, int64_t n, const uint32_t *sorted_hash, const i
     SPH_CUDA_TRY(c, cudaMemsetAsync(c->cell_mask, 0, sizeof(uint32_t) * cells, c->stream));
     owner_mask_kernel<<<div_up(div_up(n, kMaskItems), 256), 256, 0, c->stream>>>(n, sorted_hash, sorted_owner, c->cell_mask);
     SPH_CHECK_LAUNCH(c);
-    stencil_flag_kernel<<<div_up(cells, 256), 256, 0, c->stream>>>(c->grid, c->cell_mask, cs, ce,
-                                                                   c->cell_flag_count);
+    {
+        const int64_t groups = (int64_t)((c->grid.nx + kFlagCells - 1) / kFlagCells) * c->grid.ny * c->grid.nz;
+        stencil_flag_kernel<<<div_up(groups, 256), 256, 0, c->stream>>>(c->grid, c->cell_mask, cs, ce,
+                                                                        c->cell_flag_count);
+    }
     SPH_CHECK_LAUNCH(c);
     int rc = launch_scan_exclusive(c, cells, c->cell_flag_count, c->cell_offset, boundary_count);
     if (rc != SPH_OK) return rc;
