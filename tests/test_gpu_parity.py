@@ -261,3 +261,18 @@ def test_pack_boundary_matches_oracle(sph, oracle, make):
     np.testing.assert_array_equal(packed.owner.cpu().numpy(), ref.owner)
     np.testing.assert_array_equal(np.diff(ref.offsets.astype(np.int64)), parity.u32(out.owner_counts))
     ctx.close()
+
+
+@pytest.mark.parametrize("scale", [0.93, 0.8], ids=["window-borderline", "window-overflow"])
+def test_denser_packing_exercises_the_fallback_paths(sph, oracle, scale):
+    """The tiled interaction kernel holds at most kCap window records and 640 table entries per
+    bucket; denser regions fall back to the direct walk (whole tile, or single bucket).  Half of
+    the block is compressed towards x = 0 so that tiled, borderline and fallback tiles coexist."""
+    import dataclasses
+    w = wl.t1b(side=22, seed=1103)
+    posm = w.posm.copy()
+    left = posm[:, 0] < 11.0
+    posm[left, :3] *= np.float32(scale)               # denser on the left, unchanged lattice on the right
+    w2 = dataclasses.replace(w, posm=posm, name=f"dense{scale}")
+    rep = parity.lockstep(sph, oracle, w2, steps=2)
+    assert rep[-1]["pairs"] > 0
