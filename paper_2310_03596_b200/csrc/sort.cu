@@ -128,7 +128,8 @@ template <bool FIRST>
 __global__ void __launch_bounds__(kSortThreads, 2)
 onesweep_kernel(int64_t n, const uint32_t *__restrict__ keys_in, const uint32_t *__restrict__ vals_in,
                 uint32_t *__restrict__ keys_out, uint32_t *__restrict__ vals_out,
-                const uint32_t *__restrict__ hist_excl, uint32_t *status, uint32_t *ticket, int shift)
+                const uint32_t *__restrict__ hist_excl, uint32_t *status, uint32_t *ticket, int shift,
+                uint32_t *__restrict__ inv_out /* optional: inv_out[value] = destination */)
 {
     extern __shared__ __align__(16) unsigned char sort_smem_raw[];
     SortSmem &sm = *reinterpret_cast<SortSmem *>(sort_smem_raw);
@@ -276,8 +277,10 @@ onesweep_kernel(int64_t n, const uint32_t *__restrict__ keys_in, const uint32_t 
             const uint32_t kk = sm.keys[p];
             const uint32_t dg = (kk >> shift) & (kRadix - 1);
             const uint32_t dst = sm.gbase[dg] + (uint32_t)p;
+            const uint32_t vv = sm.vals[p];
             keys_out[dst] = kk;
-            vals_out[dst] = sm.vals[p];
+            vals_out[dst] = vv;
+            if (inv_out) inv_out[vv] = dst;
         }
     }
 }
@@ -334,11 +337,11 @@ int launch_sort(sph_ctx *c, int64_t n, const uint32_t *hash, uint32_t *sorted_ha
         if (p == 0)
             onesweep_kernel<true><<<(unsigned)tiles, kSortThreads, sizeof(SortSmem), c->stream>>>(
                 n, kin, vin, kout, vout, c->hist + p * kRadix, status, c->tile_counter + p,
-                p * kRadixBits);
+                p * kRadixBits, nullptr);
         else
             onesweep_kernel<false><<<(unsigned)tiles, kSortThreads, sizeof(SortSmem), c->stream>>>(
                 n, kin, vin, kout, vout, c->hist + p * kRadix, status, c->tile_counter + p,
-                p * kRadixBits);
+                p * kRadixBits, nullptr);
         SPH_CHECK_LAUNCH(c);
         kin = kout;
         vin = vout;
@@ -367,13 +370,16 @@ __global__ void segment_offsets_kernel(const uint32_t *__restrict__ hist_excl, i
 }
 
 int launch_partition_by_label(sph_ctx *c, int64_t m, const uint32_t *ids, const int32_t *label, int n_labels,
-                              uint32_t *offsets, uint32_t *ids_out)
+                              uint32_t *offsets, uint32_t *dest)
 {
+    // dest[k] = position of list entry k in the label-segmented order (a SCATTER map: the caller
+    // then reads the list and the records in list order, which is sector-friendly, and writes
+    // n_labels sequential streams -- the gather form re-read every sector once per label)
     if (m == 0) {
         SPH_CUDA_TRY(c, cudaMemsetAsync(offsets, 0, sizeof(uint32_t) * (n_labels + 1), c->stream));
         return SPH_OK;
     }
-    uint32_t *key = c->alt_keys, *key_out = c->alt_vals;      // scratch of the sort (stream-ordered)
+    uint32_t *key = c->alt_keys, *key_out = c->alt_vals, *val_out = c->s_comm_hash;  // scratch (stream-ordered)
     const int64_t tiles = (m + kSortTile - 1) / kSortTile;
     SPH_CUDA_TRY(c, cudaMemsetAsync(c->hist, 0, sizeof(uint32_t) * kRadix, c->stream));
     SPH_CUDA_TRY(c, cudaMemsetAsync(c->tile_counter, 0, sizeof(uint32_t), c->stream));
@@ -388,10 +394,11 @@ int launch_partition_by_label(sph_ctx *c, int64_t m, const uint32_t *ids, const 
     SPH_CHECK_LAUNCH(c);
     segment_offsets_kernel<<<1, 64, 0, c->stream>>>(c->hist, n_labels, (uint32_t)m, offsets);
     SPH_CHECK_LAUNCH(c);
-    SPH_CUDA_TRY(c, cudaFuncSetAttribute(onesweep_kernel<false>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+    SPH_CUDA_TRY(c, cudaFuncSetAttribute(onesweep_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize,
                                          (int)sizeof(SortSmem)));
-    onesweep_kernel<false><<<(unsigned)tiles, kSortThreads, sizeof(SortSmem), c->stream>>>(
-        m, key, ids, key_out, ids_out, c->hist, c->tile_status, c->tile_counter, 0);
+    // values = the implicit list indices 0..m-1 (FIRST), so inv_out[k] is entry k's destination
+    onesweep_kernel<true><<<(unsigned)tiles, kSortThreads, sizeof(SortSmem), c->stream>>>(
+        m, key, nullptr, key_out, val_out, c->hist, c->tile_status, c->tile_counter, 0, dest);
     SPH_CHECK_LAUNCH(c);
     return SPH_OK;
 }

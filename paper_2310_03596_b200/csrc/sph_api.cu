@@ -198,10 +198,11 @@ int sph_pack_boundary(sph_ctx *c, int64_t n, int64_t m, const sph_state *state, 
 {
     if (!n_ok(c, n) || m < 0 || m > n || !state_ok(state) || !owner_offsets) return SPH_EINVAL;
     if (m > 0 && (!boundary_ids || !packed_ids || !state_ok(packed))) return SPH_EINVAL;
-    int rc = launch_partition_by_label(c, m, boundary_ids, state->owner, c->params.n_owners, owner_offsets,
-                                       packed_ids);
+    uint32_t *dest = c->s_boundary_ids;   // scratch: destination of every list entry
+    if (boundary_ids == dest) return SPH_EINVAL;
+    int rc = launch_partition_by_label(c, m, boundary_ids, state->owner, c->params.n_owners, owner_offsets, dest);
     if (rc != SPH_OK || m == 0) return rc;
-    return launch_reorder(c, m, packed_ids, state, packed);   // gather the records segment by segment
+    return launch_scatter_records(c, m, boundary_ids, dest, state, packed, packed_ids);
 }
 
 int sph_cell_ranges(sph_ctx *c, int64_t n, const uint32_t *sorted_hash, uint32_t *cs, uint32_t *ce)

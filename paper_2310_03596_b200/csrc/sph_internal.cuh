@@ -124,7 +124,9 @@ int launch_integrate(sph_ctx *c, int64_t n, float dt, const sph_state *in, const
                      const float *acc, const float *const dsig[6], const sph_state *out,
                      const uint32_t *scatter_perm /* NULL = elementwise */);
 int launch_partition_by_label(sph_ctx *c, int64_t m, const uint32_t *ids, const int32_t *label, int n_labels,
-                              uint32_t *offsets, uint32_t *ids_out);
+                              uint32_t *offsets, uint32_t *dest /* [m] scatter map */);
+int launch_scatter_records(sph_ctx *c, int64_t m, const uint32_t *ids, const uint32_t *dest,
+                           const sph_state *in, const sph_state *out, uint32_t *packed_ids);
 int launch_scan_exclusive(sph_ctx *c, int64_t n, const uint32_t *in, uint32_t *out,
                           uint32_t *total /* dev scalar */);
 
