@@ -46,6 +46,9 @@ def _load():
     lib.orc_interact.argtypes = [i64, vp, vp, vp, vp, vp, vp, vp, f32, f32, f32, i64, vp,
                                  vp, vp, vp, vp, vp]
     lib.orc_interact.restype = None
+    lib.orc_interact_split.argtypes = [i64, vp, vp, vp, vp, vp, vp, vp, f32, f32, f32, vp, C.c_int,
+                                       vp, vp, vp, vp, vp]
+    lib.orc_interact_split.restype = None
     lib.orc_integrate.argtypes = [i64, f64, vp, vp, vp, vp, vp, vp, vp, vp, vp]
     lib.orc_integrate.restype = None
     _lib = lib
@@ -188,6 +191,29 @@ def interact(posm, velr, sig, sorted_hash, dims, cell_start, cell_end, h, K, G, 
                          _p(cell_end), np.float32(h), np.float32(K), np.float32(G),
                          m if idx is not None else 0, _p(idx) if idx is not None else None,
                          _p(drho), _p(L), _p(acc), _p(dsig), C.byref(pc))
+    return Rates(drho, L, acc, dsig, int(pc.value))
+
+
+def interact_split(posm, velr, sig, sorted_hash, dims, cell_start, cell_end, h, K, G, owner, which) -> Rates:
+    """Step e alone (which = 1: same-owner neighbours) or step f alone (which = 2: other owners);
+    sph_oracle.c orc_interact_split.  All arrays in sorted order."""
+    posm = _c(posm, np.float32)
+    velr = _c(velr, np.float32)
+    sig = _c(sig, np.float32)
+    owner = _c(owner, np.int32)
+    n = posm.shape[0]
+    sorted_hash = _c(sorted_hash, np.uint32)
+    dims = _c(dims, np.int32)
+    cell_start = _c(cell_start, np.uint32)
+    cell_end = _c(cell_end, np.uint32)
+    drho = np.zeros(n, np.float64)
+    L = np.zeros((n, 3, 3), np.float64)
+    acc = np.zeros((n, 3), np.float64)
+    dsig = np.zeros((n, 6), np.float64)
+    pc = C.c_int64(0)
+    _load().orc_interact_split(n, _p(posm), _p(velr), _p(sig), _p(sorted_hash), _p(dims), _p(cell_start),
+                               _p(cell_end), np.float32(h), np.float32(K), np.float32(G), _p(owner),
+                               int(which), _p(drho), _p(L), _p(acc), _p(dsig), C.byref(pc))
     return Rates(drho, L, acc, dsig, int(pc.value))
 
 

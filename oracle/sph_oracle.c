@@ -256,10 +256,16 @@ static void orc_sym_load(const float *sig, int64_t n, int64_t k, double s[3][3])
     s[1][2] = s[2][1] = yz;
 }
 
-void orc_interact(int64_t n, const float *posm, const float *velr, const float *sig,
+/* which = 0: every neighbour (steps e and f together, the one-GPU loop);
+ * which = 1: step e alone, "local particle interaction routines" -- only neighbours
+ *            carrying the particle's own owner label;
+ * which = 2: step f alone, "local particle interaction with the MGPU boundary
+ *            particles" -- only neighbours carrying another label.
+ * The sums are linear in the pair contributions, so pass 1 + pass 2 = pass 0 up to rounding. */
+static void orc_interact_impl(int64_t n, const float *posm, const float *velr, const float *sig,
                   const uint32_t *sorted_hash, const int32_t *dims, const uint32_t *cell_start,
                   const uint32_t *cell_end, float h_f32, float K_f32, float G_f32,
-                  int64_t n_idx, const int64_t *idx,
+                  int64_t n_idx, const int64_t *idx, const int32_t *owner, int which,
                   double *drho, double *L, double *acc, double *dsig, int64_t *pair_count)
 {
     const double h = (double)h_f32, K = (double)K_f32, G = (double)G_f32;
@@ -288,6 +294,8 @@ void orc_interact(int64_t n, const float *posm, const float *velr, const float *
                     const int64_t c = x + nx * (y + ny * z);
                     for (int64_t j = cell_start[c]; j < (int64_t)cell_end[c]; ++j) {
                         if (j == i) continue; /* S15 */
+                        if (which == 1 && owner[j] != owner[i]) continue; /* step e */
+                        if (which == 2 && owner[j] == owner[i]) continue; /* step f */
                         const double xij[3] = { xi[0] - posm[4 * j + 0], xi[1] - posm[4 * j + 1],
                                                 xi[2] - posm[4 * j + 2] };
                         const double r2 = xij[0] * xij[0] + xij[1] * xij[1] + xij[2] * xij[2];
@@ -315,6 +323,8 @@ void orc_interact(int64_t n, const float *posm, const float *velr, const float *
                     const int64_t c = x + nx * (y + ny * z);
                     for (int64_t j = cell_start[c]; j < (int64_t)cell_end[c]; ++j) {
                         if (j == i) continue;
+                        if (which == 1 && owner[j] != owner[i]) continue;
+                        if (which == 2 && owner[j] == owner[i]) continue;
                         const double xij[3] = { xi[0] - posm[4 * j + 0], xi[1] - posm[4 * j + 1],
                                                 xi[2] - posm[4 * j + 2] };
                         const double r2 = xij[0] * xij[0] + xij[1] * xij[1] + xij[2] * xij[2];
@@ -359,6 +369,27 @@ void orc_interact(int64_t n, const float *posm, const float *velr, const float *
         dsig[6 * out + 3] = sd[0][1]; dsig[6 * out + 4] = sd[0][2]; dsig[6 * out + 5] = sd[1][2];
     }
     if (pair_count) *pair_count = pairs;
+}
+
+void orc_interact(int64_t n, const float *posm, const float *velr, const float *sig,
+                  const uint32_t *sorted_hash, const int32_t *dims, const uint32_t *cell_start,
+                  const uint32_t *cell_end, float h_f32, float K_f32, float G_f32,
+                  int64_t n_idx, const int64_t *idx,
+                  double *drho, double *L, double *acc, double *dsig, int64_t *pair_count)
+{
+    orc_interact_impl(n, posm, velr, sig, sorted_hash, dims, cell_start, cell_end, h_f32, K_f32, G_f32,
+                      n_idx, idx, NULL, 0, drho, L, acc, dsig, pair_count);
+}
+
+/* NEXT-3: steps e (which = 1) and f (which = 2) as separate passes; owner is in sorted order. */
+void orc_interact_split(int64_t n, const float *posm, const float *velr, const float *sig,
+                        const uint32_t *sorted_hash, const int32_t *dims, const uint32_t *cell_start,
+                        const uint32_t *cell_end, float h_f32, float K_f32, float G_f32,
+                        const int32_t *owner, int which,
+                        double *drho, double *L, double *acc, double *dsig, int64_t *pair_count)
+{
+    orc_interact_impl(n, posm, velr, sig, sorted_hash, dims, cell_start, cell_end, h_f32, K_f32, G_f32,
+                      0, NULL, owner, which, drho, L, acc, dsig, pair_count);
 }
 
 /* ------------------------------------------------------------------------------------------

@@ -492,3 +492,37 @@ def test_pack_boundary_single_owner_is_empty():
                  floats=False)
     pb = orc.pack_boundary(r.boundary_ids, w.owner, w.n_owners, w.posm, w.velr, w.sig)
     assert pb.ids.size == 0 and (pb.offsets == 0).all()
+
+
+# ----------------------------------------------------------------------------- NEXT-3: split passes
+def test_split_passes_sum_to_the_single_pass_and_match_bruteforce():
+    """Steps e and f as separate passes: pass e + pass f = the single pass (the
+    sums are linear in the pair contributions), pair counts add up, and pass f alone equals a
+    dense O(N^2) evaluation restricted to pairs with different owners."""
+    w = W.t1b(side=10, seed=1104)
+    owner = (np.arange(w.n) % 3).astype(np.int32)         # thoroughly mixed labels
+    r = orc.step(w.posm, w.velr, w.sig, owner, w.origin, w.dims, w.h, w.K, w.G, 3, w.dt, floats=False)
+    p = r.perm
+    sp, sv, ss, so = w.posm[p], w.velr[p], np.ascontiguousarray(w.sig[:, p]), owner[p]
+    args = (sp, sv, ss, r.sorted_hash, w.dims, r.cell_start, r.cell_end, w.h, w.K, w.G)
+    full = orc.interact(*args)
+    e = orc.interact_split(*args, so, 1)
+    f = orc.interact_split(*args, so, 2)
+    assert e.pair_count + f.pair_count == full.pair_count and e.pair_count > 0 and f.pair_count > 0
+    for name in ("drho", "acc", "dsig", "L"):
+        a, b, c = getattr(e, name), getattr(f, name), getattr(full, name)
+        assert np.max(np.abs(a + b - c)) <= 1e-13 * max(np.max(np.abs(c)), 1e-300), name
+    # dense evaluation of the other-owner pairs only (momentum part: sigma_i term included per pair)
+    x = sp[:, :3].astype(np.float64); m = sp[:, 3].astype(np.float64)
+    v = sv[:, :3].astype(np.float64); rho = sv[:, 3].astype(np.float64)
+    h = float(w.h)
+    xij = x[:, None, :] - x[None, :, :]
+    rr = np.sqrt((xij ** 2).sum(-1))
+    nb = (rr < 2 * h) & ~np.eye(w.n, dtype=bool) & (so[:, None] != so[None, :])
+    alpha = 21.0 / (16.0 * np.pi * h ** 3)
+    Fm = np.where(nb, -(5.0 * alpha / h ** 2) * (1 - rr / (2 * h)) ** 3, 0.0)
+    gW = Fm[..., None] * xij
+    vij = v[:, None, :] - v[None, :, :]
+    drho = (m[None, :] * (vij * gW).sum(-1)).sum(1)
+    np.testing.assert_allclose(f.drho, drho, rtol=0, atol=1e-12 * np.max(np.abs(drho)))
+    assert f.pair_count == int(nb.sum())
