@@ -128,6 +128,17 @@ int sph_interact(sph_ctx *ctx, int64_t n, const sph_state *sorted, const uint32_
                  const uint32_t *cell_start, const uint32_t *cell_end, float *drho, float *acc,
                  float *const dsig[6], unsigned long long *pair_count);
 
+/* NEXT-3 -- steps e and f of the paper as SEPARATE passes ("local
+ * particle interaction routines", overlapped with the broadcast; "local particle
+ * interaction with the MGPU boundary particles"): which = 1 takes only the neighbours that carry
+ * the particle's own owner label (step e), which = 2 only those with another label (step f).
+ * Same arguments and outputs as sph_interact; the rates are linear in the pair contributions, so
+ * pass 1 + pass 2 equals sph_interact up to rounding, and the pair counts add up exactly
+ * (pair_count accumulates; zero it first).  sorted->owner is read. */
+int sph_interact_split(sph_ctx *ctx, int64_t n, const sph_state *sorted, const uint32_t *sorted_hash,
+                       const uint32_t *cell_start, const uint32_t *cell_end, int32_t which,
+                       float *drho, float *acc, float *const dsig[6], unsigned long long *pair_count);
+
 /* Stage 4b -- explicit integration, symplectic Euler (step g; reading S18):
  * rho += dt drho; v += dt acc; sigma += dt dsig; x += dt v(new).  m and owner are copied.
  * Elementwise: in, rates and out use the same index order; out may alias in. */

@@ -8,13 +8,14 @@ namespace sphb {
 int launch_interact(sph_ctx *c, int64_t n, const sph_state *sorted, const uint32_t *sorted_hash,
                     const uint32_t *cs, const uint32_t *ce, float *drho, float *acc,
                     float *const dsig[6], unsigned long long *pair_count, const sph_state *fuse_out,
-                    const uint32_t *perm, float dt)
+                    const uint32_t *perm, float dt, int mode)
 {
     if (n == 0) return SPH_OK;
     InteractIn in;
     InteractOut out;
     in.posm = reinterpret_cast<const float4 *>(sorted->posm);
     in.velr = reinterpret_cast<const float4 *>(sorted->velr);
+    in.owner = sorted->owner;
     out.drho = drho;   // NULL (with fuse_out set): the rates are not stored
     out.acc = reinterpret_cast<float4 *>(acc);
     for (int i = 0; i < 6; ++i) { in.sig[i] = sorted->sig[i]; out.dsig[i] = dsig ? dsig[i] : nullptr; }
@@ -29,8 +30,8 @@ int launch_interact(sph_ctx *c, int64_t n, const sph_state *sorted, const uint32
         for (int i = 0; i < 6; ++i) out.o_sig[i] = fuse_out->sig[i];
     }
     if (c->params.flags & SPH_FLAG_INTERACT_DIRECT)
-        return launch_interact_direct(c, n, in, sorted_hash, cs, ce, out, pair_count);
-    return launch_interact_tiled(c, n, in, sorted_hash, cs, ce, out, pair_count);
+        return launch_interact_direct(c, n, in, sorted_hash, cs, ce, out, pair_count, mode);
+    return launch_interact_tiled(c, n, in, sorted_hash, cs, ce, out, pair_count, mode);
 }
 
 }  // namespace sphb

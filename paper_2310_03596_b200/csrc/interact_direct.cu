@@ -13,14 +13,14 @@ namespace sphb {
 __global__ void __launch_bounds__(128)
 interact_direct_kernel(int64_t n, InteractIn in, const uint32_t *__restrict__ sorted_hash,
                        const uint32_t *__restrict__ cs, const uint32_t *__restrict__ ce, Grid g,
-                       Consts k, InteractOut out, unsigned long long *pair_count)
+                       Consts k, InteractOut out, unsigned long long *pair_count, int mode)
 {
     const int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
     unsigned long long my_pairs = 0;
     if (i < n) {
         const uint32_t h = sorted_hash[i];
         const int cx = h % g.nx, cy = (h / g.nx) % g.ny, cz = h / (g.nx * g.ny);
-        my_pairs = direct_particle(i, cx, cy, cz, in, cs, ce, g, k, out);
+        my_pairs = direct_particle(i, cx, cy, cz, in, cs, ce, g, k, out, mode);
     }
     if (pair_count) {
         // warp, then one atomic per warp
@@ -32,10 +32,10 @@ interact_direct_kernel(int64_t n, InteractIn in, const uint32_t *__restrict__ so
 
 int launch_interact_direct(sph_ctx *c, int64_t n, const InteractIn &in, const uint32_t *sorted_hash,
                            const uint32_t *cs, const uint32_t *ce, const InteractOut &out,
-                           unsigned long long *pair_count)
+                           unsigned long long *pair_count, int mode)
 {
     interact_direct_kernel<<<div_up(n, 128), 128, 0, c->stream>>>(n, in, sorted_hash, cs, ce, c->grid,
-                                                                  c->consts, out, pair_count);
+                                                                  c->consts, out, pair_count, mode);
     SPH_CHECK_LAUNCH(c);
     return SPH_OK;
 }

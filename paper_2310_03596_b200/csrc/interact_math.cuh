@@ -14,7 +14,12 @@ namespace sphb {
 struct InteractIn {
     const float4 *posm, *velr;
     const float *sig[6];
+    const int32_t *owner;   // sorted owner labels; only read by the split passes (NEXT-3)
 };
+
+// Which neighbours a pass takes: 0 = all (steps e and f as one loop),
+// 1 = step e alone (same owner label), 2 = step f alone (other owner labels).
+constexpr int kPassAll = 0, kPassLocal = 1, kPassRemote = 2;
 struct InteractOut {
     float *drho;          // rates, indexed by sorted position; all three NULL = not wanted
     float4 *acc;
@@ -262,8 +267,10 @@ __device__ __forceinline__ void finish_particle(const PairAccum &A, const float 
 __device__ __forceinline__ uint32_t direct_particle(int64_t i, int cx, int cy, int cz,
                                                     const InteractIn &in, const uint32_t *__restrict__ cs,
                                                     const uint32_t *__restrict__ ce, const Grid &g,
-                                                    const Consts &k, const InteractOut &out)
+                                                    const Consts &k, const InteractOut &out,
+                                                    int mode = kPassAll)
 {
+    const int32_t oi = mode != kPassAll ? in.owner[i] : 0;
     const float4 pi = in.posm[i];
     const float4 vi = in.velr[i];
     PairAccum A;
@@ -282,6 +289,7 @@ __device__ __forceinline__ uint32_t direct_particle(int64_t i, int cx, int cy, i
                 const float4 pj = in.posm[j];
                 const float dx = pi.x - pj.x, dy_ = pi.y - pj.y, dz_ = pi.z - pj.z;
                 const float r2 = dx * dx + dy_ * dy_ + dz_ * dz_;
+                if (mode != kPassAll && ((in.owner[j] == oi) != (mode == kPassLocal))) continue;
                 if (r2 < k.support2 && j != (uint32_t)i) {
                     const float4 vj = in.velr[j];
                     const float inv_rho = 1.0f / vj.w;
@@ -306,9 +314,9 @@ __device__ __forceinline__ uint32_t direct_particle(int64_t i, int cx, int cy, i
 
 int launch_interact_direct(sph_ctx *c, int64_t n, const InteractIn &in, const uint32_t *sorted_hash,
                            const uint32_t *cs, const uint32_t *ce, const InteractOut &out,
-                           unsigned long long *pair_count);
+                           unsigned long long *pair_count, int mode);
 int launch_interact_tiled(sph_ctx *c, int64_t n, const InteractIn &in, const uint32_t *sorted_hash,
                           const uint32_t *cs, const uint32_t *ce, const InteractOut &out,
-                          unsigned long long *pair_count);
+                          unsigned long long *pair_count, int mode);
 
 }  // namespace sphb

@@ -128,6 +128,7 @@ struct __align__(16) TileSmem {
     int bkt_tsm[kNB];         // shared-memory record index of its first target
     uint32_t bkt_tb0[kNB];    // sorted index of its first target
     uint64_t bar;
+    uint8_t own[kCap + 8];    // owner label of every window record (split passes only, NEXT-3)
 };
 
 // ------------------------------------------------------------------------------------ kernel
@@ -177,7 +178,7 @@ __device__ __forceinline__ float4 ld_rec(const float4 *base, uint32_t e16)
     return *reinterpret_cast<const float4 *>(reinterpret_cast<const char *>(base) + e16);
 }
 
-template <bool kCount>
+template <bool kCount, int kMode>
 __global__ void __launch_bounds__(kTW * 32, 2)
 interact_tiled_kernel(Packed rec, InteractIn in, const uint32_t *__restrict__ cs,
                       const uint32_t *__restrict__ ce, Grid g, Consts k, InteractOut out,
@@ -234,7 +235,7 @@ interact_tiled_kernel(Packed rec, InteractIn in, const uint32_t *__restrict__ cs
     if (total > kCap) {
         // window too large for shared memory (very dense region): direct walk, warp = bucket
         for (int i = lane; i < nt; i += 32)
-            my_pairs += direct_particle((int64_t)tb0 + i, cxb, cyb, cz, in, cs, ce, g, k, out);
+            my_pairs += direct_particle((int64_t)tb0 + i, cxb, cyb, cz, in, cs, ce, g, k, out, kMode);
     } else {
         __syncthreads();  // mbarrier initialised before the copies are issued against it
         if (warp == 0) {
@@ -312,6 +313,14 @@ interact_tiled_kernel(Packed rec, InteractIn in, const uint32_t *__restrict__ cs
                 pa.w = pa.x * pa.x + pa.y * pa.y + pa.z * pa.z;   // the mass travels in D.z
                 sm.A[j] = pa;
             }
+            if (kMode != kPassAll) {
+                // owner labels of the window records, run by run (lane r of every warp describes run r)
+                for (int r = 0; r < kRuns; ++r) {
+                    const int lo = __shfl_sync(0xffffffffu, run_lo, r), off = __shfl_sync(0xffffffffu, run_off, r);
+                    const int len = __shfl_sync(0xffffffffu, run_len, r);
+                    for (int i = tid; i < len; i += kTW * 32) sm.own[off + i] = (uint8_t)in.owner[lo + i];
+                }
+            }
             if (tid < 8) {
                 sm.A[kDummy + tid] = make_float4(1e18f, 1e18f, 1e18f, 3e36f);
                 sm.B[kDummy + tid] = make_float4(0.f, 0.f, 0.f, 0.f);
@@ -324,7 +333,7 @@ interact_tiled_kernel(Packed rec, InteractIn in, const uint32_t *__restrict__ cs
         // a bucket whose table overflowed is walked directly by its own warp
         if (nt > 0 && sm.cand_len[warp] < 0)
             for (int i = lane; i < nt; i += 32)
-                my_pairs += direct_particle((int64_t)tb0 + i, cxb, cyb, cz, in, cs, ce, g, k, out);
+                my_pairs += direct_particle((int64_t)tb0 + i, cxb, cyb, cz, in, cs, ce, g, k, out, kMode);
 
         // ---- work units: lane b < kNB keeps the record of bucket b -----------------------------
         int l_nt = 0, l_tsm = 0, l_wp = 0, l_ng = 0;
@@ -381,27 +390,52 @@ interact_tiled_kernel(Packed rec, InteractIn in, const uint32_t *__restrict__ cs
                 az23 = __shfl_xor_sync(0xffffffffu, az01, 16); nt23 = __shfl_xor_sync(0xffffffffu, nt01, 16);
             }
 
+            // split passes: owner labels of the 4 slots, one byte each (0xFF = absent target)
+            uint32_t own4 = 0;
+            if (kMode != kPassAll) {
+                const uint32_t o0 = my_valid ? (uint32_t)sm.own[tbase + my_t] : 0xFFu;
+                const uint32_t o1 = __shfl_xor_sync(0xffffffffu, o0, 8);
+                const uint32_t o01 = o0 | (o1 << 8);
+                own4 = o01 | (__shfl_xor_sync(0xffffffffu, o01, 16) << 16);
+            }
+            // keeps, of the 4 fresh mask bits of one candidate, those the pass takes:
+            // same-owner pairs (step e) or other-owner pairs (step f)
+            auto owner_filter = [&](uint32_t &mask, uint32_t e) {
+                if (kMode == kPassAll) return;
+                const uint32_t oj = sm.own[e >> 4];
+                uint32_t eq = 0;
+#pragma unroll
+                for (int dd = 0; dd < 4; ++dd) eq |= (((own4 >> (8 * dd)) & 0xFFu) == oj ? 1u : 0u) << dd;
+                mask &= ~0xFu | (kMode == kPassLocal ? eq : ~eq);
+            };
+
             // ---- phase 1: the whole table, bit 4 s + d of mask word s / 8 <- chunk s, slot d ----
             uint32_t m0 = 0, m1 = 0, m2 = 0;
             const int nch = Wp >> 5;
             const uint16_t *cb = cand + lane;
 #pragma unroll 1
             for (int s = nch - 1; s >= 16; --s) {
-                const float4 pa = ld_rec(sm.A, cb[32 * s]);
+                const uint32_t ce_ = cb[32 * s];
+                const float4 pa = ld_rec(sm.A, ce_);
                 test_push2(m2, pa, ax23, ay23, az23, nt23);
                 test_push2(m2, pa, ax01, ay01, az01, nt01);
+                owner_filter(m2, ce_);
             }
 #pragma unroll 4
             for (int s = min(nch, 16) - 1; s >= 8; --s) {
-                const float4 pa = ld_rec(sm.A, cb[32 * s]);
+                const uint32_t ce_ = cb[32 * s];
+                const float4 pa = ld_rec(sm.A, ce_);
                 test_push2(m1, pa, ax23, ay23, az23, nt23);
                 test_push2(m1, pa, ax01, ay01, az01, nt01);
+                owner_filter(m1, ce_);
             }
 #pragma unroll 4
             for (int s = min(nch, 8) - 1; s >= 0; --s) {
-                const float4 pa = ld_rec(sm.A, cb[32 * s]);
+                const uint32_t ce_ = cb[32 * s];
+                const float4 pa = ld_rec(sm.A, ce_);
                 test_push2(m0, pa, ax23, ay23, az23, nt23);
                 test_push2(m0, pa, ax01, ay01, az01, nt01);
+                owner_filter(m0, ce_);
             }
             // every quarter collects the bits of its own target: slot d of the lanes of quarter
             // q ^ d.  Afterwards bit beta of word w <-> table position 256 w + t + 8 (beta ^ q).
@@ -484,7 +518,7 @@ interact_tiled_kernel(Packed rec, InteractIn in, const uint32_t *__restrict__ cs
                     row[17] = __int_as_float(tbase + my_t);
                 }
             }
-            if (my_valid && t == 0) ++my_self;  // the self pair is not a pair (reading S15)
+            if (kMode != kPassRemote && my_valid && t == 0) ++my_self;  // the self pair is not a pair (reading S15)
             ++parked;
             if (parked == kSlots / 4 || gi + kTW >= NG) {
                 // ---- epilogue: one lane per parked target (O8, stores) ------------------------
@@ -554,7 +588,7 @@ interact_tiled_kernel(Packed rec, InteractIn in, const uint32_t *__restrict__ cs
 
 int launch_interact_tiled(sph_ctx *c, int64_t n, const InteractIn &in, const uint32_t *sorted_hash,
                           const uint32_t *cs, const uint32_t *ce, const InteractOut &out,
-                          unsigned long long *pair_count)
+                          unsigned long long *pair_count, int mode)
 {
     (void)sorted_hash;
     Packed rec;
@@ -570,21 +604,38 @@ int launch_interact_tiled(sph_ctx *c, int64_t n, const InteractIn &in, const uin
     static bool attr_set = false;
     const int smem = (int)sizeof(TileSmem);
     if (!attr_set) {
-        SPH_CUDA_TRY(c, cudaFuncSetAttribute(interact_tiled_kernel<true>,
+        SPH_CUDA_TRY(c, cudaFuncSetAttribute(interact_tiled_kernel<true, kPassAll>,
                                              cudaFuncAttributeMaxDynamicSharedMemorySize, smem));
-        SPH_CUDA_TRY(c, cudaFuncSetAttribute(interact_tiled_kernel<false>,
+        SPH_CUDA_TRY(c, cudaFuncSetAttribute(interact_tiled_kernel<false, kPassAll>,
+                                             cudaFuncAttributeMaxDynamicSharedMemorySize, smem));
+        SPH_CUDA_TRY(c, cudaFuncSetAttribute(interact_tiled_kernel<true, kPassLocal>,
+                                             cudaFuncAttributeMaxDynamicSharedMemorySize, smem));
+        SPH_CUDA_TRY(c, cudaFuncSetAttribute(interact_tiled_kernel<true, kPassRemote>,
                                              cudaFuncAttributeMaxDynamicSharedMemorySize, smem));
         attr_set = true;
     }
     const int tiles_x = (c->grid.nx + kTBX - 1) / kTBX, tiles_y = (c->grid.ny + kTBY - 1) / kTBY;
     const int64_t tiles = (int64_t)tiles_x * tiles_y * c->grid.nz;
     if (tiles > 0x7fffffffll) return SPH_EINVAL;
-    if (pair_count)
-        interact_tiled_kernel<true><<<(unsigned)tiles, kTW * 32, smem, c->stream>>>(
-            rec, in, cs, ce, c->grid, c->consts, out, pair_count, tiles_x, tiles_y);
-    else
-        interact_tiled_kernel<false><<<(unsigned)tiles, kTW * 32, smem, c->stream>>>(
-            rec, in, cs, ce, c->grid, c->consts, out, pair_count, tiles_x, tiles_y);
+    const unsigned gr = (unsigned)tiles;
+    if (mode == kPassAll) {
+        if (pair_count)
+            interact_tiled_kernel<true, kPassAll><<<gr, kTW * 32, smem, c->stream>>>(
+                rec, in, cs, ce, c->grid, c->consts, out, pair_count, tiles_x, tiles_y);
+        else
+            interact_tiled_kernel<false, kPassAll><<<gr, kTW * 32, smem, c->stream>>>(
+                rec, in, cs, ce, c->grid, c->consts, out, pair_count, tiles_x, tiles_y);
+    } else {
+        // the split passes always count (one instantiation each); without a caller buffer the
+        // count goes to ctx scratch
+        unsigned long long *pc = pair_count ? pair_count : c->s_pair_count;
+        if (mode == kPassLocal)
+            interact_tiled_kernel<true, kPassLocal><<<gr, kTW * 32, smem, c->stream>>>(
+                rec, in, cs, ce, c->grid, c->consts, out, pc, tiles_x, tiles_y);
+        else
+            interact_tiled_kernel<true, kPassRemote><<<gr, kTW * 32, smem, c->stream>>>(
+                rec, in, cs, ce, c->grid, c->consts, out, pc, tiles_x, tiles_y);
+    }
     SPH_CHECK_LAUNCH(c);
     return SPH_OK;
 }

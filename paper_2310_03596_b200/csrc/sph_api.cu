@@ -235,6 +235,18 @@ int sph_interact(sph_ctx *c, int64_t n, const sph_state *sorted, const uint32_t 
     return launch_interact(c, n, sorted, sorted_hash, cs, ce, drho, acc, dsig, pair_count, nullptr, nullptr, 0.f);
 }
 
+int sph_interact_split(sph_ctx *c, int64_t n, const sph_state *sorted, const uint32_t *sorted_hash,
+                       const uint32_t *cs, const uint32_t *ce, int32_t which, float *drho, float *acc,
+                       float *const dsig[6], unsigned long long *pair_count)
+{
+    if (!n_ok(c, n) || !state_ok(sorted) || !sorted_hash || !cs || !ce || !drho || !acc || !dsig) return SPH_EINVAL;
+    if (which != 1 && which != 2) return SPH_EINVAL;
+    for (int i = 0; i < 6; ++i)
+        if (!dsig[i]) return SPH_EINVAL;
+    return launch_interact(c, n, sorted, sorted_hash, cs, ce, drho, acc, dsig, pair_count, nullptr, nullptr, 0.f,
+                           which);
+}
+
 int sph_integrate(sph_ctx *c, int64_t n, float dt, const sph_state *in, const float *drho,
                   const float *acc, const float *const dsig[6], const sph_state *out)
 {

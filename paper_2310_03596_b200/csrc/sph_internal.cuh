@@ -119,7 +119,8 @@ int launch_comm_hash(sph_ctx *c, int64_t n, const uint32_t *sorted_hash, const i
 int launch_interact(sph_ctx *c, int64_t n, const sph_state *sorted, const uint32_t *sorted_hash,
                     const uint32_t *cs, const uint32_t *ce, float *drho, float *acc,
                     float *const dsig[6], unsigned long long *pair_count,
-                    const sph_state *fuse_out /* NULL = rates only */, const uint32_t *perm, float dt);
+                    const sph_state *fuse_out /* NULL = rates only */, const uint32_t *perm, float dt,
+                    int mode = 0 /* 0 all, 1 same-owner, 2 other-owner neighbours */);
 int launch_integrate(sph_ctx *c, int64_t n, float dt, const sph_state *in, const float *drho,
                      const float *acc, const float *const dsig[6], const sph_state *out,
                      const uint32_t *scatter_perm /* NULL = elementwise */);

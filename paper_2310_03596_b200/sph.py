@@ -29,7 +29,7 @@ FLAG_INTERACT_DIRECT = 1
 EXPORTS = (
     "sph_create", "sph_destroy", "sph_hash", "sph_sort", "sph_reorder", "sph_cell_ranges",
     "sph_comm_hash", "sph_interact", "sph_integrate", "sph_step", "sph_step_host", "sph_pack_boundary",
-    "sph_enable_timing", "sph_get_timing", "sph_launch_count", "sph_strerror",
+    "sph_interact_split", "sph_enable_timing", "sph_get_timing", "sph_launch_count", "sph_strerror",
     "sph_last_cuda_error",
 )
 
@@ -70,6 +70,7 @@ def load_library() -> C.CDLL:
     lib.sph_cell_ranges.argtypes = [vp, i64, vp, vp, vp]
     lib.sph_comm_hash.argtypes = [vp, i64] + [vp] * 9
     lib.sph_interact.argtypes = [vp, i64, sp, vp, vp, vp, vp, vp, C.POINTER(vp * 6), vp]
+    lib.sph_interact_split.argtypes = [vp, i64, sp, vp, vp, vp, i32, vp, vp, C.POINTER(vp * 6), vp]
     lib.sph_integrate.argtypes = [vp, i64, f32, sp, vp, vp, C.POINTER(vp * 6), sp]
     lib.sph_step.argtypes = [vp, i64, f32, sp] + [vp] * 11 + [C.POINTER(vp * 6), vp]
     lib.sph_step_host.argtypes = [vp, i64, f32, i32, sp, vp, vp, vp]
@@ -298,6 +299,19 @@ class Context:
                                         acc.data_ptr(), C.byref(d6), pc.data_ptr()), "sph_interact")
         return drho, acc, dsig, pc
 
+    def sph_interact_split(self, sorted_state: State, sorted_hash, cell_start, cell_end, which: int):
+        """Step e alone (which = 1, same-owner neighbours) or step f alone (which = 2)."""
+        n = sorted_state.n
+        drho, acc, dsig = self._f32(n), self._f32(n, 4), self._f32(6, n)
+        pc = torch.zeros(1, dtype=torch.int64, device=self.device)
+        s = sorted_state._c()
+        d6 = _six(dsig)
+        self._chk(self.lib.sph_interact_split(self.handle, n, C.byref(s), sorted_hash.data_ptr(),
+                                              cell_start.data_ptr(), cell_end.data_ptr(), int(which),
+                                              drho.data_ptr(), acc.data_ptr(), C.byref(d6), pc.data_ptr()),
+                  "sph_interact_split")
+        return drho, acc, dsig, pc
+
     def sph_integrate(self, dt, state: State, drho, acc, dsig, out: State | None = None) -> State:
         n = state.n
         out = out if out is not None else State.empty(n, self.device)
@@ -366,6 +380,7 @@ def sph_reorder(ctx, *a, **k): return ctx.sph_reorder(*a, **k)
 def sph_cell_ranges(ctx, *a, **k): return ctx.sph_cell_ranges(*a, **k)
 def sph_comm_hash(ctx, *a, **k): return ctx.sph_comm_hash(*a, **k)
 def sph_interact(ctx, *a, **k): return ctx.sph_interact(*a, **k)
+def sph_interact_split(ctx, *a, **k): return ctx.sph_interact_split(*a, **k)
 def sph_integrate(ctx, *a, **k): return ctx.sph_integrate(*a, **k)
 def sph_step(ctx, *a, **k): return ctx.sph_step(*a, **k)
 def sph_step_host(ctx, *a, **k): return ctx.sph_step_host(*a, **k)

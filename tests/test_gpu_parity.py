@@ -276,3 +276,51 @@ def test_denser_packing_exercises_the_fallback_paths(sph, oracle, scale):
     w2 = dataclasses.replace(w, posm=posm, name=f"dense{scale}")
     rep = parity.lockstep(sph, oracle, w2, steps=2)
     assert rep[-1]["pairs"] > 0
+
+
+# ------------------------------------------------------------------ NEXT-3: steps e and f as separate passes
+@pytest.mark.parametrize("flags", [0, 1], ids=["tiled", "direct"])
+@pytest.mark.parametrize("make", [lambda: wl.t1b(side=18, seed=1105), lambda: wl.config(2, side=33)],
+                         ids=["t1b-mixed-owners", "cfg2"])
+def test_split_passes_match_oracle_and_sum_to_single_pass(sph, oracle, make, flags):
+    """sph_interact_split: each pass against oracle.interact_split at 1e-5 (per
+    field, normalised by the SINGLE pass's field maximum), pair counts exact-ish (S25), and pass e +
+    pass f against sph_interact."""
+    w = make()
+    owner = w.owner if w.n_owners > 2 else (np.arange(w.n) % 5).astype(np.int32)
+    n_owners = max(w.n_owners, 5)
+    ctx = sph.Context(w.origin, w.dims, w.h, w.K, w.G, n_owners=n_owners, max_n=w.n, flags=flags)
+    state = sph.State.from_numpy(w.posm, w.velr, w.sig, owner)
+    h = ctx.sph_hash(state.posm)
+    sh, perm = ctx.sph_sort(h)
+    st = ctx.sph_reorder(perm, state)
+    cs, ce = ctx.sph_cell_ranges(sh)
+    full = ctx.sph_interact(st, sh, cs, ce)
+    torch.cuda.synchronize()
+    p = parity.u32(perm)
+    sp, sv, ss, so = w.posm[p], w.velr[p], np.ascontiguousarray(w.sig[:, p]), owner[p]
+    args = (sp, sv, ss, parity.u32(sh), w.dims, parity.u32(cs), parity.u32(ce), w.h, w.K, w.G)
+    ref_full = oracle.interact(*args)
+    scale = {"drho": np.max(np.abs(ref_full.drho)), "acc": np.max(np.abs(ref_full.acc)),
+             "dsig": np.max(np.abs(ref_full.dsig))}
+    total = [0.0, 0.0, 0.0]
+    pairs = 0
+    for which in (1, 2):
+        drho, acc, dsig, pc = ctx.sph_interact_split(st, sh, cs, ce, which)
+        torch.cuda.synchronize()
+        ref = oracle.interact_split(*args, so, which)
+        g = {"drho": drho.cpu().numpy(), "acc": acc.cpu().numpy()[:, :3], "dsig": dsig.cpu().numpy().T}
+        r = {"drho": ref.drho, "acc": ref.acc, "dsig": ref.dsig}
+        for k_ in g:
+            dif = np.max(np.abs(g[k_] - r[k_]))
+            err = dif / scale[k_] if scale[k_] > 0 else (0.0 if dif < 1e-30 else np.inf)   # S21
+            assert err <= parity.RATE_TOL, (which, k_, err)
+        assert abs(int(pc.cpu()[0]) - ref.pair_count) <= max(1e-6 * ref.pair_count, 2)
+        pairs += int(pc.cpu()[0])
+        total = [total[0] + g["drho"], total[1] + g["acc"], total[2] + g["dsig"]]
+    gf = [full[0].cpu().numpy(), full[1].cpu().numpy()[:, :3], full[2].cpu().numpy().T]
+    for t_, f_, k_ in zip(total, gf, ("drho", "acc", "dsig")):
+        dif = np.max(np.abs(t_ - f_))
+        assert (dif / scale[k_] if scale[k_] > 0 else (0.0 if dif < 1e-30 else np.inf)) <= parity.RATE_TOL, k_
+    assert abs(pairs - int(full[3].cpu()[0])) <= 4
+    ctx.close()
