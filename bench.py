@@ -271,6 +271,36 @@ def run_ours(args, rank, world, local_rank):
                 "note": "includes the allocation of the output tensors by the binding"}
         del o2, bids_dev, bcnt
 
+    # ---- NEXT-3 (not part of the step metric): steps e / f as separate interaction passes ----
+    split = None
+    if w.n_owners > 1:
+        hh = ctx.sph_hash(state.posm)
+        sh_, pm_ = ctx.sph_sort(hh)
+        st_ = ctx.sph_reorder(pm_, state)
+        cs_, ce_ = ctx.sph_cell_ranges(sh_)
+
+        def _t(fn):
+            ts = []
+            for _ in range(4):
+                flush.zero_()
+                a_, b_ = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+                a_.record()
+                r_ = fn()
+                b_.record()
+                torch.cuda.synchronize(dev)
+                ts.append(a_.elapsed_time(b_))
+            return float(np.median(ts[1:])), r_
+
+        t_all, r_all = _t(lambda: ctx.sph_interact(st_, sh_, cs_, ce_))
+        t_e, r_e = _t(lambda: ctx.sph_interact_split(st_, sh_, cs_, ce_, 1))
+        t_f, r_f = _t(lambda: ctx.sph_interact_split(st_, sh_, cs_, ce_, 2))
+        split = {"single_pass_ms": round(t_all, 4), "pass_e_ms": round(t_e, 4), "pass_f_ms": round(t_f, 4),
+                 "pairs_single": int(r_all[3].cpu()[0]), "pairs_e": int(r_e[3].cpu()[0]),
+                 "pairs_f": int(r_f[3].cpu()[0]),
+                 "note": "stand-alone sph_interact calls (pack pass and output allocation included)"}
+        del hh, sh_, pm_, st_, cs_, ce_, r_all, r_e, r_f
+
+    # ---- end to end through the C-ABI with pinned host buffers ----
     host = sph.State.from_numpy(w.posm, w.velr, w.sig, w.owner, device="cpu", pin=True)
     bids = torch.empty(n, dtype=torch.int32).pin_memory().numpy().view(np.uint32)
     ctx.sph_step_host(host, w.dt, 1, bids)               # warm-up (allocates staging)
@@ -340,6 +370,8 @@ def run_ours(args, rank, world, local_rank):
         pack["gbs"] = round(pack["bytes_per_boundary_particle"] * pack["boundary_particles"] / (pack["ms"] * 1e-3) / 1e9, 1)
         pack["hbm_frac"] = round(pack["gbs"] / peaks["hbm_gbs"], 3)
         line["next1_pack_boundary"] = pack
+    if split:
+        line["next3_split_passes"] = split
     if world == 1 and not args.no_cpu_baseline:
         cb = time_oracle(w, args.cpu_sample, 3, 1)
         line["cpu_baseline"] = {k_: cb[k_] for k_ in ("value", "unit", "cores", "kind", "sample")}
