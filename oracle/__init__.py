@@ -39,6 +39,8 @@ def _load():
     lib.orc_boundary.restype = i64
     lib.orc_pack_boundary.argtypes = [i64, i64, vp, vp, C.c_int32] + [vp] * 9
     lib.orc_pack_boundary.restype = None
+    lib.orc_balance.argtypes = [i64, vp, vp, C.c_int32, C.c_int32, vp]
+    lib.orc_balance.restype = i64
     lib.orc_kernel_W.argtypes = [f64, f64]
     lib.orc_kernel_W.restype = f64
     lib.orc_kernel_F.argtypes = [f64, f64]
@@ -124,6 +126,19 @@ def boundary(comm_hash_, perm, sorted_owner, n_owners: int):
     if m < 0:
         raise MemoryError("orc_boundary")
     return ids[:m].copy(), counts
+
+
+def balance(posm, owner, n_owners: int, hmax: int = 1000):
+    """One sweep of the paper's communication-load balancing over all owner pairs (sph_oracle.c
+    O10).  Returns (new owner labels, number of swapped pairs, balancing hash of the
+    last pair that touched each particle)."""
+    posm = _c(posm, np.float32)
+    own = np.array(owner, dtype=np.int32, copy=True)
+    bh = np.zeros(posm.shape[0], np.int32)
+    k = _load().orc_balance(posm.shape[0], _p(posm), _p(own), int(n_owners), int(hmax), _p(bh))
+    if k < 0:
+        raise MemoryError("orc_balance")
+    return own, int(k), bh
 
 
 @dataclass

@@ -415,3 +415,106 @@ void orc_integrate(int64_t n, double dt, const float *posm, const float *velr, c
             sig_out[(int64_t)c * n + i] = (double)sig[(int64_t)c * n + i] + dt * dsig[6 * i + c];
     }
 }
+
+/* ------------------------------------------------------------------------------------------
+ * O10  Communication-load balancing, single particle type (
+ * PAPER.md:36, section III.A), followed step by step, one sweep over all owner pairs:
+ *   "Every GPU computes its own particle cloud centre of gravity (Cg).  A balancing hash number
+ *    is defined based on the projection of the particle position on the line from one GPU Cg
+ *    to the other.  If the projection is located on the own GPU side of the middle of the
+ *    segment of the two Cgs, the particle is disregarded for swapping (hash number 0).  If the
+ *    projection is located beyond the other Cg, the particle is given the maximum swapping hash
+ *    number (typically 1000).  In between the balancing hash number is proportional to the
+ *    distance between the middle of the Cgs and the other Cg up to the maximum swapping hash
+ *    number.  If both GPUs have particles with positive hash numbers, some particle swapping
+ *    occurs.  The number of particles to be swapped is determined by the minimum number of
+ *    particles with a positive hash number on each GPU.  The particle data can be sorted by the
+ *    balancing hash number and the corresponding particles can be swapped between the two GPUs.
+ *    The algorithm is then repeated for each GPU pair."
+ * Readings: B1 pairs (A, B), A < B, in lexicographic order, labels
+ * updated after every pair, Cgs recomputed before every pair; B2 Cg = unweighted mean position,
+ * summed EXACTLY in 2^-16 fixed point (int64), so that the result does not depend on the order of
+ * the reduction; B3 s = ((x - CgA) . d) / (d . d), d = CgB - CgA, fp64, sums left to right, no
+ * contraction; B4 hash = 0 if !(s > 1/2), hmax if s >= 1, else ceil(hmax (2 s - 1)) clipped to
+ * [1, hmax]; B5 a pair with an empty owner or coincident Cgs is skipped; B6 n = min(nA, nB), the
+ * n particles of each side that come first in the order (hash descending, id ascending) swap
+ * labels; B7 hmax = 1000 by default.
+ * owner [n] is updated in place; bal_hash (may be NULL) receives, for the LAST pair processed
+ * that involved the particle, its balancing hash (diagnostic).  Returns the number of swapped
+ * particle pairs.
+ * ---------------------------------------------------------------------------------------- */
+typedef struct { int32_t hash; uint32_t id; } orc_bal;
+
+static int orc_bal_cmp(const void *a, const void *b)
+{
+    const orc_bal *x = (const orc_bal *)a, *y = (const orc_bal *)b;
+    if (x->hash != y->hash) return x->hash > y->hash ? -1 : 1; /* hash descending */
+    if (x->id != y->id) return x->id < y->id ? -1 : 1;         /* id ascending (B6) */
+    return 0;
+}
+
+static int32_t orc_balance_hash(const float *posm, int64_t i, const double cg_own[3],
+                                const double cg_other[3], int32_t hmax)
+{
+    const double d0 = cg_other[0] - cg_own[0], d1 = cg_other[1] - cg_own[1], d2 = cg_other[2] - cg_own[2];
+    const double dd = d0 * d0 + d1 * d1 + d2 * d2;
+    const double e0 = (double)posm[4 * i + 0] - cg_own[0], e1 = (double)posm[4 * i + 1] - cg_own[1],
+                 e2 = (double)posm[4 * i + 2] - cg_own[2];
+    const double s = (e0 * d0 + e1 * d1 + e2 * d2) / dd;
+    if (!(s > 0.5)) return 0;
+    if (s >= 1.0) return hmax;
+    double hv = ceil((double)hmax * (2.0 * s - 1.0));
+    if (hv < 1.0) hv = 1.0;
+    if (hv > (double)hmax) hv = (double)hmax;
+    return (int32_t)hv;
+}
+
+int64_t orc_balance(int64_t n, const float *posm, int32_t *owner, int32_t n_owners, int32_t hmax,
+                    int32_t *bal_hash)
+{
+    orc_bal *la = (orc_bal *)malloc((size_t)(n > 0 ? n : 1) * sizeof(orc_bal));
+    orc_bal *lb = (orc_bal *)malloc((size_t)(n > 0 ? n : 1) * sizeof(orc_bal));
+    if (!la || !lb) { free(la); free(lb); return -1; }
+    int64_t swapped = 0;
+    for (int32_t A = 0; A < n_owners; ++A)
+        for (int32_t B = A + 1; B < n_owners; ++B) {
+            int64_t sum[2][3] = { { 0, 0, 0 }, { 0, 0, 0 } }, cnt[2] = { 0, 0 };
+            for (int64_t i = 0; i < n; ++i) {
+                const int side = owner[i] == A ? 0 : (owner[i] == B ? 1 : -1);
+                if (side < 0) continue;
+                for (int a = 0; a < 3; ++a) sum[side][a] += (int64_t)llrint((double)posm[4 * i + a] * 65536.0);
+                cnt[side] += 1;
+            }
+            if (cnt[0] == 0 || cnt[1] == 0) continue; /* B5 */
+            double cg[2][3];
+            for (int side = 0; side < 2; ++side)
+                for (int a = 0; a < 3; ++a)
+                    cg[side][a] = ((double)sum[side][a] / (double)cnt[side]) * (1.0 / 65536.0);
+            if (cg[0][0] == cg[1][0] && cg[0][1] == cg[1][1] && cg[0][2] == cg[1][2]) continue; /* B5 */
+            int64_t na = 0, nb = 0;
+            for (int64_t i = 0; i < n; ++i) {
+                if (owner[i] == A) {
+                    const int32_t hv = orc_balance_hash(posm, i, cg[0], cg[1], hmax);
+                    if (bal_hash) bal_hash[i] = hv;
+                    if (hv > 0) { la[na].hash = hv; la[na].id = (uint32_t)i; ++na; }
+                } else if (owner[i] == B) {
+                    const int32_t hv = orc_balance_hash(posm, i, cg[1], cg[0], hmax);
+                    if (bal_hash) bal_hash[i] = hv;
+                    if (hv > 0) { lb[nb].hash = hv; lb[nb].id = (uint32_t)i; ++nb; }
+                }
+            }
+            const int64_t m = na < nb ? na : nb;
+            if (m == 0) continue;
+            qsort(la, (size_t)na, sizeof(orc_bal), orc_bal_cmp);
+            qsort(lb, (size_t)nb, sizeof(orc_bal), orc_bal_cmp);
+            for (int64_t k = 0; k < m; ++k) {
+                owner[la[k].id] = B;
+                owner[lb[k].id] = A;
+            }
+            swapped += m;
+        }
+    free(la);
+    free(lb);
+    return swapped;
+}
+

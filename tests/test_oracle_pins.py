@@ -526,3 +526,75 @@ def test_split_passes_sum_to_the_single_pass_and_match_bruteforce():
     drho = (m[None, :] * (vij * gW).sum(-1)).sum(1)
     np.testing.assert_allclose(f.drho, drho, rtol=0, atol=1e-12 * np.max(np.abs(drho)))
     assert f.pair_count == int(nb.sum())
+
+
+# ----------------------------------------------------------------------------- NEXT-2: balancing
+def test_balance_hand_worked_example_golden():
+    """PAPER.md:36 on four particles, worked by hand (tests/golden/balancing_worked_example.txt)."""
+    rows = [l.split() for l in open(os.path.join(GOLDEN, "balancing_worked_example.txt"))
+            if l.strip() and not l.startswith("#")]
+    x = np.array([float(r[1]) for r in rows], np.float32)
+    posm = np.zeros((len(rows), 4), np.float32); posm[:, 0] = x; posm[:, 3] = 1
+    own0 = np.array([int(r[2]) for r in rows], np.int32)
+    own, k, bh = orc.balance(posm, own0, 2)
+    assert k == 1
+    np.testing.assert_array_equal(bh, [int(r[3]) for r in rows])
+    np.testing.assert_array_equal(own, [int(r[4]) for r in rows])
+
+
+def test_balance_keeps_counts_slabs_are_a_fixed_point_single_owner_noop():
+    """'The computational workload will stay balanced for all the swapping operations'
+    (PAPER.md:30): every swap exchanges one particle each way; a slab decomposition has no
+    particle past the middle of any Cg pair, so nothing moves."""
+    w = W.lattice_block(24, 24, 24, 0.1, 21, owners=("random", 5))
+    own, k, _ = orc.balance(w.posm, w.owner, 5)
+    assert k > 0
+    np.testing.assert_array_equal(np.bincount(own, minlength=5), np.bincount(w.owner, minlength=5))
+    w1 = W.config(1, side=32)
+    own1, k1, _ = orc.balance(w1.posm, w1.owner, w1.n_owners)
+    assert k1 == 0 and np.array_equal(own1, w1.owner)
+    w2 = W.lattice_block(10, 10, 10, 0.1, 22, owners=("single",))
+    own2, k2, _ = orc.balance(w2.posm, w2.owner, 1)
+    assert k2 == 0 and (own2 == 0).all()
+
+
+def test_balance_hash_against_independent_projection():
+    """One pair, dense numpy: projection on the Cg-Cg line, 0 on the own side of the middle,
+    hmax beyond the other Cg, proportional in between; swap count = min of the
+    positive counts; the swapped particles are the ones with the largest hashes."""
+    rng = np.random.default_rng(5)
+    n = 400
+    posm = np.ones((n, 4), np.float32); posm[:, :3] = rng.random((n, 3), dtype=np.float32) * 10
+    own0 = (rng.random(n) < 0.5).astype(np.int32)
+    own, k, bh = orc.balance(posm, own0, 2)
+    x = posm[:, :3].astype(np.float64)
+    cg = [x[own0 == g].mean(0) for g in (0, 1)]
+    h = np.zeros(n, np.int64)
+    for g in (0, 1):
+        d = cg[1 - g] - cg[g]
+        s = ((x - cg[g]) @ d) / (d @ d)
+        hv = np.where(s >= 1, 1000, np.where(s > 0.5, np.clip(np.ceil(1000 * (2 * s - 1)), 1, 1000), 0))
+        h[own0 == g] = hv[own0 == g]
+    assert np.mean(bh == h) > 0.995              # fixed-point Cg vs fp64 mean: a few ceil() flips at most
+    na, nb = int(((bh > 0) & (own0 == 0)).sum()), int(((bh > 0) & (own0 == 1)).sum())
+    assert k == min(na, nb)
+    moved = own != own0
+    assert moved.sum() == 2 * k and (bh[moved] > 0).all()
+    for g in (0, 1):                              # the movers of a side have the largest hashes of that side
+        side = own0 == g
+        if (side & moved).any() and (side & ~moved & (bh > 0)).any():
+            assert bh[side & moved].min() >= bh[side & ~moved].max()
+
+
+def test_balance_restores_a_compact_decomposition():
+    """The Fig. 1 -> Fig. 2 effect (PAPER.md:38 'the information exchange subset is always close
+    to a surface'): random labels make every particle a boundary particle; a few sweeps bring the
+    boundary fraction down towards that of a slab decomposition."""
+    w = W.lattice_block(40, 40, 40, 0.1, 78, owners=("random", 3))
+    own = w.owner
+    for _ in range(3):
+        own, _, _ = orc.balance(w.posm, own, 3)
+    r = orc.step(w.posm, w.velr, w.sig, own, w.origin, w.dims, w.h, w.K, w.G, 3, w.dt, floats=False)
+    assert r.boundary_ids.size < 0.55 * w.n
+    r0 = orc.step(w.posm, w.velr, w.sig, w.owner, w.origin, w.dims, w.h, w.K, w.G, 3, w.dt, floats=False)
+    assert r0.boundary_ids.size == w.n
