@@ -180,6 +180,23 @@ int sph_pack_boundary(sph_ctx *ctx, int64_t n, int64_t m, const sph_state *state
                       const uint32_t *boundary_ids, uint32_t *owner_offsets, uint32_t *packed_ids,
                       const sph_state *packed);
 
+/* NEXT-2 -- one sweep of the communication-load balancing heuristic on the owner
+ * labels, single particle type (section III.A; the paper runs it every 20 integration
+ * loops, PAPER.md:32 -- the cadence is the caller's).  For every owner pair (A, B), A < B, in
+ * lexicographic order (labels and centres of gravity are updated after every pair): Cg = unweighted
+ * mean position of an owner's particles; balancing hash of a particle = 0 if its projection s on
+ * the line Cg_own -> Cg_other (s = 0 at Cg_own, 1 at Cg_other) is not beyond the middle (s <= 1/2),
+ * hmax if s >= 1, else ceil(hmax (2 s - 1)); n = min over the two owners of the number of particles
+ * with a positive hash; the n first particles of each side in the order (hash descending, id
+ * ascending) swap labels.  Every owner keeps its particle count.  Exact arithmetic contract (so
+ * that the labels have one correct value): Cg from 2^-16 fixed-point int64 coordinate sums, s in
+ * fp64 without contraction.
+ * In: posm dev [n][4] in id order; hmax in 1 .. 1023 (the paper's typical value: 1000).
+ * In/out: owner dev [n].  Out (optional, may be NULL): bal_hash dev [n] = the hash each particle
+ * got in the last pair that involved it (0 if none); swapped dev scalar = particle pairs swapped. */
+int sph_balance(sph_ctx *ctx, int64_t n, const float *posm, int32_t *owner, int32_t hmax,
+                int32_t *bal_hash, unsigned long long *swapped);
+
 /* End-to-end variant with HOST buffers (pinned memory recommended): uploads the id-ordered state,
  * runs `steps` iterations, downloads the state, the boundary list of the last step and the
  * counters, and synchronises the stream before returning.  Device staging lives in the ctx

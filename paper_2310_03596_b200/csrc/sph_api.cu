@@ -68,6 +68,7 @@ void carve(sph_ctx *c, char *base, size_t *total)
     c->rec_B = k.take<float4>(n + 2);
     c->rec_C = k.take<float4>(n + 2);
     c->rec_D = k.take<float4>(n + 2);
+    c->bal = k.take<unsigned long long>((balance_scratch_bytes() + 7) / 8);
     *total = align_up(k.off, 256);
 }
 
@@ -203,6 +204,13 @@ int sph_pack_boundary(sph_ctx *c, int64_t n, int64_t m, const sph_state *state, 
     int rc = launch_partition_by_label(c, m, boundary_ids, state->owner, c->params.n_owners, owner_offsets, dest);
     if (rc != SPH_OK || m == 0) return rc;
     return launch_scatter_records(c, m, boundary_ids, dest, state, packed, packed_ids);
+}
+
+int sph_balance(sph_ctx *c, int64_t n, const float *posm, int32_t *owner, int32_t hmax, int32_t *bal_hash,
+                unsigned long long *swapped)
+{
+    if (!n_ok(c, n) || !posm || !owner || hmax < 1 || hmax > 1023) return SPH_EINVAL;
+    return launch_balance(c, n, posm, owner, hmax, bal_hash, swapped);
 }
 
 int sph_cell_ranges(sph_ctx *c, int64_t n, const uint32_t *sorted_hash, uint32_t *cs, uint32_t *ce)

@@ -81,6 +81,7 @@ struct sph_ctx {
     sph_state sorted;                         // sorted copy of the state
     float4 *rec_B, *rec_C;                    // packed neighbour records of the interaction kernel
     float4 *rec_D;
+    void *bal;                                // control block of the balancing sweep (balance.cu)
     bool rec_fresh;                           // rec_B/C/D already hold the records of `sorted` (written by reorder)
     // host-API staging (lazy)
     sph_state staging;
@@ -128,6 +129,9 @@ int launch_partition_by_label(sph_ctx *c, int64_t m, const uint32_t *ids, const 
                               uint32_t *offsets, uint32_t *dest /* [m] scatter map */);
 int launch_scatter_records(sph_ctx *c, int64_t m, const uint32_t *ids, const uint32_t *dest,
                            const sph_state *in, const sph_state *out, uint32_t *packed_ids);
+int launch_balance(sph_ctx *c, int64_t n, const float *posm, int32_t *owner, int hmax, int32_t *bal_hash,
+                   unsigned long long *swapped);
+size_t balance_scratch_bytes();
 int launch_scan_exclusive(sph_ctx *c, int64_t n, const uint32_t *in, uint32_t *out,
                           uint32_t *total /* dev scalar */);
 

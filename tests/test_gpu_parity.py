@@ -324,3 +324,30 @@ def test_split_passes_match_oracle_and_sum_to_single_pass(sph, oracle, make, fla
         assert (dif / scale[k_] if scale[k_] > 0 else (0.0 if dif < 1e-30 else np.inf)) <= parity.RATE_TOL, k_
     assert abs(pairs - int(full[3].cpu()[0])) <= 4
     ctx.close()
+
+
+# ------------------------------------------------------------------ NEXT-2: balancing sweep
+@pytest.mark.parametrize("make,g", [(lambda: wl.lattice_block(24, 24, 24, 0.1, 21, owners=("random", 5)), 5),
+                                    (lambda: wl.lattice_block(30, 26, 22, 0.1, 23, owners=("slabs_mixed", 3, 0.1)), 3),
+                                    (lambda: wl.config(1, side=32), 4),
+                                    (lambda: wl.config(4, side=20), 16),
+                                    (lambda: wl.lattice_block(9, 9, 9, 0.1, 24, owners=("single",)), 1)],
+                         ids=["random5", "mixed3", "slabs-fixed-point", "random16", "one-owner"])
+def test_balance_sweep_matches_oracle_bit_exact(sph, oracle, make, g):
+    """sph_balance against oracle.balance: labels, balancing hashes and the swap count
+    are integers decided by pinned arithmetic (fixed-point Cg sums, fp64 projection without
+    contraction) -- bit-exact, over three consecutive sweeps."""
+    w = make()
+    ctx = sph.Context.for_workload(w)
+    posm = torch.from_numpy(w.posm).cuda()
+    own_gpu = torch.from_numpy(w.owner.copy()).cuda()
+    own_ref = w.owner.copy()
+    for sweep in range(3):
+        bh, sw = ctx.sph_balance(posm, own_gpu)
+        torch.cuda.synchronize()
+        own_ref, k, bh_ref = oracle.balance(w.posm, own_ref, g)
+        assert int(sw.cpu()[0]) == k, sweep
+        np.testing.assert_array_equal(bh.cpu().numpy(), bh_ref, err_msg=f"bal_hash sweep {sweep}")
+        np.testing.assert_array_equal(own_gpu.cpu().numpy(), own_ref, err_msg=f"owner sweep {sweep}")
+        np.testing.assert_array_equal(np.bincount(own_ref, minlength=g), np.bincount(w.owner, minlength=g))
+    ctx.close()
