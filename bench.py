@@ -300,6 +300,30 @@ def run_ours(args, rank, world, local_rank):
                  "note": "stand-alone sph_interact calls (pack pass and output allocation included)"}
         del hh, sh_, pm_, st_, cs_, ce_, r_all, r_e, r_f
 
+    # ---- NEXT-2 (not part of the step metric): one balancing sweep and what it does to the exchange set ----
+    bal = None
+    if 1 < w.n_owners and args.balance_sweeps > 0:
+        st_b = state.clone()
+        o_b = ctx.alloc_outputs(n)
+        ctx.sph_step(st_b.clone(), w.dt, o_b)
+        torch.cuda.synchronize(dev)
+        frac = [int(sph.as_u32(o_b.boundary_count)[0]) / n]
+        ms_b, swaps = [], []
+        for _ in range(args.balance_sweeps):
+            a_, b_ = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            a_.record()
+            _bh, sw_ = ctx.sph_balance(st_b.posm, st_b.owner)
+            b_.record()
+            torch.cuda.synchronize(dev)
+            ms_b.append(a_.elapsed_time(b_))
+            swaps.append(int(sw_.cpu()[0]))
+            ctx.sph_step(st_b.clone(), w.dt, o_b)
+            torch.cuda.synchronize(dev)
+            frac.append(int(sph.as_u32(o_b.boundary_count)[0]) / n)
+        bal = {"sweep_ms": [round(x, 3) for x in ms_b], "swapped_pairs": swaps,
+               "boundary_fraction": [round(x, 4) for x in frac], "owner_pairs": w.n_owners * (w.n_owners - 1) // 2}
+        del st_b, o_b
+
     # ---- end to end through the C-ABI with pinned host buffers ----
     host = sph.State.from_numpy(w.posm, w.velr, w.sig, w.owner, device="cpu", pin=True)
     bids = torch.empty(n, dtype=torch.int32).pin_memory().numpy().view(np.uint32)
@@ -372,6 +396,8 @@ def run_ours(args, rank, world, local_rank):
         line["next1_pack_boundary"] = pack
     if split:
         line["next3_split_passes"] = split
+    if bal:
+        line["next2_balance"] = bal
     if world == 1 and not args.no_cpu_baseline:
         cb = time_oracle(w, args.cpu_sample, 3, 1)
         line["cpu_baseline"] = {k_: cb[k_] for k_ in ("value", "unit", "cores", "kind", "sample")}
@@ -389,6 +415,7 @@ def main():
     ap.add_argument("--flags", type=int, default=0, help="sph_params.flags (1 = direct interaction kernel)")
     ap.add_argument("--stage-timing", action="store_true", help="average stage times over all steps (syncs each step)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--balance-sweeps", type=int, default=2, help="NEXT-2 report: balancing sweeps to time (0 = skip)")
     ap.add_argument("--cpu-sample", type=int, default=300000)
     ap.add_argument("--ref-sample", type=int, default=100000)
     args = ap.parse_args()

@@ -163,22 +163,40 @@ bal_swap_kernel(int64_t n, const float4 *__restrict__ posm, int32_t *__restrict_
                 const int32_t *__restrict__ bal_hash, BalCtl *ctl, int A, int B,
                 const uint32_t *__restrict__ rankA, const uint32_t *__restrict__ rankB)
 {
+    // D = (coordinates leaving A) - (coordinates leaving B): sum[A] -= D, sum[B] += D.  Exact
+    // integer sums, so the order of the block and grid reductions does not matter.
+    __shared__ long long s_d[3];
+    if (threadIdx.x < 3) s_d[threadIdx.x] = 0;
+    __syncthreads();
+    if (!ctl->valid) return;   // uniform over the grid
     const int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
-    if (i >= n || !ctl->valid) return;
-    const int o = owner[i];
-    if (o != A && o != B) return;
-    const uint32_t hv = (uint32_t)bal_hash[i];
-    const uint32_t thr = o == A ? ctl->thrA : ctl->thrB, quota = o == A ? ctl->quotaA : ctl->quotaB;
-    const uint32_t rank = o == A ? rankA[i] : rankB[i];
-    const bool move = hv > 0 && (hv > thr || (hv == thr && rank < quota));
-    if (!move) return;
-    const int to = o == A ? B : A;
-    owner[i] = to;
-    const float4 p = posm[i];
-    const long long f[3] = {fixed16(p.x), fixed16(p.y), fixed16(p.z)};
-    for (int a = 0; a < 3; ++a) {   // exact integer sums: any order
-        atomicAdd(reinterpret_cast<unsigned long long *>(&ctl->sum[o][a]), (unsigned long long)(-f[a]));
-        atomicAdd(reinterpret_cast<unsigned long long *>(&ctl->sum[to][a]), (unsigned long long)f[a]);
+    long long f[3] = {0, 0, 0};
+    if (i < n) {
+        const int o = owner[i];
+        if (o == A || o == B) {
+            const uint32_t hv = (uint32_t)bal_hash[i];
+            const uint32_t thr = o == A ? ctl->thrA : ctl->thrB, quota = o == A ? ctl->quotaA : ctl->quotaB;
+            const uint32_t rank = o == A ? rankA[i] : rankB[i];
+            if (hv > 0 && (hv > thr || (hv == thr && rank < quota))) {
+                owner[i] = o == A ? B : A;
+                const float4 p = posm[i];
+                const long long sgn = o == A ? 1 : -1;
+                f[0] = sgn * fixed16(p.x); f[1] = sgn * fixed16(p.y); f[2] = sgn * fixed16(p.z);
+            }
+        }
+    }
+#pragma unroll
+    for (int a = 0; a < 3; ++a) {
+        long long v = f[a];
+#pragma unroll
+        for (int o = 16; o > 0; o >>= 1) v += __shfl_xor_sync(0xffffffffu, v, o);
+        if ((threadIdx.x & 31) == 0 && v) atomicAdd(reinterpret_cast<unsigned long long *>(&s_d[a]), (unsigned long long)v);
+    }
+    __syncthreads();
+    if (threadIdx.x < 3 && s_d[threadIdx.x]) {
+        const long long d = s_d[threadIdx.x];
+        atomicAdd(reinterpret_cast<unsigned long long *>(&ctl->sum[A][threadIdx.x]), (unsigned long long)(-d));
+        atomicAdd(reinterpret_cast<unsigned long long *>(&ctl->sum[B][threadIdx.x]), (unsigned long long)d);
     }
 }
 
