@@ -41,6 +41,8 @@ def _load():
     lib.orc_pack_boundary.restype = None
     lib.orc_balance.argtypes = [i64, vp, vp, C.c_int32, C.c_int32, vp]
     lib.orc_balance.restype = i64
+    lib.orc_balance_types.argtypes = [i64, vp, vp, vp, C.c_int32, C.c_int32, C.c_int32, f64, vp]
+    lib.orc_balance_types.restype = i64
     lib.orc_kernel_W.argtypes = [f64, f64]
     lib.orc_kernel_W.restype = f64
     lib.orc_kernel_F.argtypes = [f64, f64]
@@ -138,6 +140,19 @@ def balance(posm, owner, n_owners: int, hmax: int = 1000):
     k = _load().orc_balance(posm.shape[0], _p(posm), _p(own), int(n_owners), int(hmax), _p(bh))
     if k < 0:
         raise MemoryError("orc_balance")
+    return own, int(k), bh
+
+
+def balance_types(posm, owner, ptype, n_owners: int, n_types: int, hmax: int = 1000, alpha: float = 0.1):
+    """Balancing sweep per particle type with the biased Cg' of PAPER.md:56 (sph_oracle.c O11)."""
+    posm = _c(posm, np.float32)
+    ptype = _c(ptype, np.int32)
+    own = np.array(owner, dtype=np.int32, copy=True)
+    bh = np.zeros(posm.shape[0], np.int32)
+    k = _load().orc_balance_types(posm.shape[0], _p(posm), _p(own), _p(ptype), int(n_owners), int(n_types),
+                                  int(hmax), float(alpha), _p(bh))
+    if k < 0:
+        raise MemoryError("orc_balance_types")
     return own, int(k), bh
 
 

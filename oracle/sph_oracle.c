@@ -518,3 +518,77 @@ int64_t orc_balance(int64_t n, const float *posm, int32_t *owner, int32_t n_owne
     return swapped;
 }
 
+/* ------------------------------------------------------------------------------------------
+ * O11  Balancing with multiple particle types (section
+ * III.B): "all particle types shall be balanced over each GPU ...  The swapping algorithm of
+ * section III.A can then be applied for each particle type.  However, this may lead to an
+ * independent decomposition from particle type to particle type.  To overcome this to a certain
+ * extent, a biased Cg' can be used ... shift the Cg used for balancing from the actual Cg of the
+ * particles of the desired type towards the global Cg of the particles:
+ *     Cg'_typeA = alpha Cg_alltypes + (1 - alpha) Cg_typeA   with alpha = 0.1".
+ * Readings: B8 types are processed in ascending order, each with the full pair sweep of O10
+ * restricted to the particles of that type (only they get a hash, only they swap); B9 Cg_alltypes
+ * of an owner is the unweighted mean over ALL its particles (current labels), Cg_type over its
+ * particles of the type, both from exact fixed-point sums; Cg' = alpha * Cg_all + (1 - alpha) *
+ * Cg_type evaluated in fp64 as written (two products, one sum, no contraction); B10 a pair is
+ * skipped when either owner holds no particle of the type or the two Cg' coincide.
+ * ---------------------------------------------------------------------------------------- */
+int64_t orc_balance_types(int64_t n, const float *posm, int32_t *owner, const int32_t *ptype,
+                          int32_t n_owners, int32_t n_types, int32_t hmax, double alpha, int32_t *bal_hash)
+{
+    orc_bal *la = (orc_bal *)malloc((size_t)(n > 0 ? n : 1) * sizeof(orc_bal));
+    orc_bal *lb = (orc_bal *)malloc((size_t)(n > 0 ? n : 1) * sizeof(orc_bal));
+    if (!la || !lb) { free(la); free(lb); return -1; }
+    int64_t swapped = 0;
+    for (int32_t T = 0; T < n_types; ++T)
+        for (int32_t A = 0; A < n_owners; ++A)
+            for (int32_t B = A + 1; B < n_owners; ++B) {
+                int64_t st[2][3] = { { 0 } }, sa[2][3] = { { 0 } }, ct[2] = { 0, 0 }, ca[2] = { 0, 0 };
+                for (int64_t i = 0; i < n; ++i) {
+                    const int side = owner[i] == A ? 0 : (owner[i] == B ? 1 : -1);
+                    if (side < 0) continue;
+                    for (int a = 0; a < 3; ++a) {
+                        const int64_t f = (int64_t)llrint((double)posm[4 * i + a] * 65536.0);
+                        sa[side][a] += f;
+                        if (ptype[i] == T) st[side][a] += f;
+                    }
+                    ca[side] += 1;
+                    if (ptype[i] == T) ct[side] += 1;
+                }
+                if (ct[0] == 0 || ct[1] == 0) continue; /* B10 */
+                double cg[2][3];
+                for (int side = 0; side < 2; ++side)
+                    for (int a = 0; a < 3; ++a) {
+                        const double call = ((double)sa[side][a] / (double)ca[side]) * (1.0 / 65536.0);
+                        const double ctyp = ((double)st[side][a] / (double)ct[side]) * (1.0 / 65536.0);
+                        cg[side][a] = alpha * call + (1.0 - alpha) * ctyp;
+                    }
+                if (cg[0][0] == cg[1][0] && cg[0][1] == cg[1][1] && cg[0][2] == cg[1][2]) continue;
+                int64_t na = 0, nb = 0;
+                for (int64_t i = 0; i < n; ++i) {
+                    if (ptype[i] != T) continue;
+                    if (owner[i] == A) {
+                        const int32_t hv = orc_balance_hash(posm, i, cg[0], cg[1], hmax);
+                        if (bal_hash) bal_hash[i] = hv;
+                        if (hv > 0) { la[na].hash = hv; la[na].id = (uint32_t)i; ++na; }
+                    } else if (owner[i] == B) {
+                        const int32_t hv = orc_balance_hash(posm, i, cg[1], cg[0], hmax);
+                        if (bal_hash) bal_hash[i] = hv;
+                        if (hv > 0) { lb[nb].hash = hv; lb[nb].id = (uint32_t)i; ++nb; }
+                    }
+                }
+                const int64_t m = na < nb ? na : nb;
+                if (m == 0) continue;
+                qsort(la, (size_t)na, sizeof(orc_bal), orc_bal_cmp);
+                qsort(lb, (size_t)nb, sizeof(orc_bal), orc_bal_cmp);
+                for (int64_t k = 0; k < m; ++k) {
+                    owner[la[k].id] = B;
+                    owner[lb[k].id] = A;
+                }
+                swapped += m;
+            }
+    free(la);
+    free(lb);
+    return swapped;
+}
+

@@ -598,3 +598,46 @@ def test_balance_restores_a_compact_decomposition():
     assert r.boundary_ids.size < 0.55 * w.n
     r0 = orc.step(w.posm, w.velr, w.sig, w.owner, w.origin, w.dims, w.h, w.K, w.G, 3, w.dt, floats=False)
     assert r0.boundary_ids.size == w.n
+
+
+# ----------------------------------------------------------------------------- NEXT-4: multi-type balancing
+def test_balance_types_formula_counts_and_limits():
+    """PAPER.md:56 Cg' = alpha Cg_all + (1 - alpha) Cg_type, alpha = 0.1:
+      * every (owner, type) count is kept (only same-type particles swap);
+      * alpha = 0 with ONE type is exactly the single-type algorithm of section III.A;
+      * alpha = 1 uses the all-type Cg for every type (same lines for both types);
+      * a hand-checkable pair: the biased centres are the alpha-blend of numpy means."""
+    rng = np.random.default_rng(9)
+    n = 600
+    posm = np.ones((n, 4), np.float32); posm[:, :3] = rng.random((n, 3), dtype=np.float32) * 12
+    owner = rng.integers(0, 3, n).astype(np.int32)
+    ptype = (rng.random(n) < 0.3).astype(np.int32)
+    own, k, bh = orc.balance_types(posm, owner, ptype, 3, 2)
+    assert k > 0
+    for t in (0, 1):
+        np.testing.assert_array_equal(np.bincount(own[ptype == t], minlength=3),
+                                      np.bincount(owner[ptype == t], minlength=3))
+    # one type, alpha = 0  ==  section III.A
+    own_a, k_a, bh_a = orc.balance(posm, owner, 3)
+    own_b, k_b, bh_b = orc.balance_types(posm, owner, np.zeros(n, np.int32), 3, 1, alpha=0.0)
+    assert k_a == k_b and np.array_equal(own_a, own_b) and np.array_equal(bh_a, bh_b)
+    # two owners only (so that exactly one pair runs per type): the type-0 hashes of owner 0 follow
+    # from numpy means blended with alpha = 0.1, written out independently of the oracle
+    keep = owner < 2
+    pm, ow, pt = posm[keep], owner[keep], ptype[keep]
+    _, _, bh2 = orc.balance_types(pm, ow, pt, 2, 2)
+    xs = pm[:, :3].astype(np.float64)
+    cg2 = [0.1 * xs[ow == g].mean(0) + 0.9 * xs[(ow == g) & (pt == 0)].mean(0) for g in (0, 1)]
+    d2 = cg2[1] - cg2[0]
+    sel2 = (ow == 0) & (pt == 0)
+    s2 = ((xs[sel2] - cg2[0]) @ d2) / (d2 @ d2)
+    e2 = np.where(s2 >= 1, 1000, np.where(s2 > 0.5, np.clip(np.ceil(1000 * (2 * s2 - 1)), 1, 1000), 0))
+    assert np.mean(bh2[sel2] == e2) > 0.99          # fixed-point Cg vs fp64 mean: a ceil() flip at most
+    # alpha = 1: both types are balanced along the same (all-type) Cg line of a pair
+    _, _, bh3 = orc.balance_types(pm, ow, pt, 2, 2, alpha=1.0)
+    cg3 = [xs[ow == g].mean(0) for g in (0, 1)]
+    d3 = cg3[1] - cg3[0]
+    sel3 = (ow == 0) & (pt == 0)                     # type 0 runs first: labels still the input's
+    s3 = ((xs[sel3] - cg3[0]) @ d3) / (d3 @ d3)
+    e3 = np.where(s3 >= 1, 1000, np.where(s3 > 0.5, np.clip(np.ceil(1000 * (2 * s3 - 1)), 1, 1000), 0))
+    assert np.mean(bh3[sel3] == e3) > 0.99
