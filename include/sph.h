@@ -197,6 +197,18 @@ int sph_pack_boundary(sph_ctx *ctx, int64_t n, int64_t m, const sph_state *state
 int sph_balance(sph_ctx *ctx, int64_t n, const float *posm, int32_t *owner, int32_t hmax,
                 int32_t *bal_hash, unsigned long long *swapped);
 
+/* NEXT-4 -- the balancing sweep for multiple particle types (PAPER.md:54-57,
+ * section III.B): the pair sweep of sph_balance is applied to each particle type in ascending
+ * order (only particles of the type get a hash and swap, so every (owner, type) count is kept),
+ * with the biased centre of gravity of PAPER.md:56
+ *     Cg'_type = alpha Cg_alltypes + (1 - alpha) Cg_type        (the paper: alpha = 0.1)
+ * where Cg_alltypes is the mean over ALL particles of the owner and Cg_type over its particles of
+ * the type (exact fixed-point sums; the blend in fp64 as written, no contraction).
+ * ptype dev [n], values in [0, n_types), n_types <= 8; 0 <= alpha <= 1; the rest as sph_balance. */
+int sph_balance_types(sph_ctx *ctx, int64_t n, const float *posm, int32_t *owner, const int32_t *ptype,
+                      int32_t n_types, double alpha, int32_t hmax, int32_t *bal_hash,
+                      unsigned long long *swapped);
+
 /* End-to-end variant with HOST buffers (pinned memory recommended): uploads the id-ordered state,
  * runs `steps` iterations, downloads the state, the boundary list of the last step and the
  * counters, and synchronises the stream before returning.  Device staging lives in the ctx

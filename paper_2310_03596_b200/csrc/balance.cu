@@ -21,9 +21,11 @@ namespace sphb {
 constexpr int kBalBins = 1024;  // hash values 0 .. hmax <= 1023
 
 // device control block of a sweep (lives in ctx->bal)
+constexpr int kBalTypes = 8;    // particle types of the multi-type variant
+
 struct BalCtl {
-    long long sum[SPH_MAX_OWNERS][3];   // fixed-point coordinate sums per owner
-    unsigned long long cnt[SPH_MAX_OWNERS];
+    long long sum[SPH_MAX_OWNERS][kBalTypes][3];   // fixed-point coordinate sums per owner and type
+    unsigned long long cnt[SPH_MAX_OWNERS][kBalTypes];
     unsigned long long swapped;         // pairs of particles swapped so far
     // per pair:
     double cgA[3], cgB[3];
@@ -38,40 +40,55 @@ __device__ __forceinline__ long long fixed16(float x)
 }
 
 __global__ void __launch_bounds__(256)
-bal_sums_kernel(int64_t n, const float4 *__restrict__ posm, const int32_t *__restrict__ owner, BalCtl *ctl)
+bal_sums_kernel(int64_t n, const float4 *__restrict__ posm, const int32_t *__restrict__ owner,
+                const int32_t *__restrict__ ptype, BalCtl *ctl)
 {
-    __shared__ long long s_sum[SPH_MAX_OWNERS][3];
-    __shared__ unsigned long long s_cnt[SPH_MAX_OWNERS];
-    for (int i = threadIdx.x; i < SPH_MAX_OWNERS * 3; i += blockDim.x) (&s_sum[0][0])[i] = 0;
-    if (threadIdx.x < SPH_MAX_OWNERS) s_cnt[threadIdx.x] = 0;
+    __shared__ long long s_sum[SPH_MAX_OWNERS][kBalTypes][3];
+    __shared__ unsigned long long s_cnt[SPH_MAX_OWNERS][kBalTypes];
+    for (int i = threadIdx.x; i < SPH_MAX_OWNERS * kBalTypes * 3; i += blockDim.x) (&s_sum[0][0][0])[i] = 0;
+    for (int i = threadIdx.x; i < SPH_MAX_OWNERS * kBalTypes; i += blockDim.x) (&s_cnt[0][0])[i] = 0;
     __syncthreads();
     for (int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += (int64_t)gridDim.x * blockDim.x) {
         const float4 p = posm[i];
         const int o = owner[i] & (SPH_MAX_OWNERS - 1);
-        atomicAdd(reinterpret_cast<unsigned long long *>(&s_sum[o][0]), (unsigned long long)fixed16(p.x));
-        atomicAdd(reinterpret_cast<unsigned long long *>(&s_sum[o][1]), (unsigned long long)fixed16(p.y));
-        atomicAdd(reinterpret_cast<unsigned long long *>(&s_sum[o][2]), (unsigned long long)fixed16(p.z));
-        atomicAdd(&s_cnt[o], 1ull);
+        const int t = ptype ? (ptype[i] & (kBalTypes - 1)) : 0;
+        atomicAdd(reinterpret_cast<unsigned long long *>(&s_sum[o][t][0]), (unsigned long long)fixed16(p.x));
+        atomicAdd(reinterpret_cast<unsigned long long *>(&s_sum[o][t][1]), (unsigned long long)fixed16(p.y));
+        atomicAdd(reinterpret_cast<unsigned long long *>(&s_sum[o][t][2]), (unsigned long long)fixed16(p.z));
+        atomicAdd(&s_cnt[o][t], 1ull);
     }
     __syncthreads();
-    for (int i = threadIdx.x; i < SPH_MAX_OWNERS * 3; i += blockDim.x)
-        if ((&s_sum[0][0])[i])
-            atomicAdd(reinterpret_cast<unsigned long long *>(&ctl->sum[0][0]) + i, (unsigned long long)(&s_sum[0][0])[i]);
-    if (threadIdx.x < SPH_MAX_OWNERS && s_cnt[threadIdx.x]) atomicAdd(&ctl->cnt[threadIdx.x], s_cnt[threadIdx.x]);
+    for (int i = threadIdx.x; i < SPH_MAX_OWNERS * kBalTypes * 3; i += blockDim.x)
+        if ((&s_sum[0][0][0])[i])
+            atomicAdd(reinterpret_cast<unsigned long long *>(&ctl->sum[0][0][0]) + i,
+                      (unsigned long long)(&s_sum[0][0][0])[i]);
+    for (int i = threadIdx.x; i < SPH_MAX_OWNERS * kBalTypes; i += blockDim.x)
+        if ((&s_cnt[0][0])[i]) atomicAdd(&ctl->cnt[0][0] + i, (&s_cnt[0][0])[i]);
 }
 
 // one thread: centres of gravity of the pair, validity, cleared histograms
-__global__ void bal_pair_begin_kernel(BalCtl *ctl, int A, int B)
+__global__ void bal_pair_begin_kernel(BalCtl *ctl, int A, int B, int T, int typed, double alpha)
 {
     for (int i = threadIdx.x; i < 2 * kBalBins; i += blockDim.x) (&ctl->hist[0][0])[i] = 0;
     if (threadIdx.x != 0) return;
-    const unsigned long long ca = ctl->cnt[A], cb = ctl->cnt[B];
-    int valid = ca != 0 && cb != 0;
+    const unsigned long long ca = ctl->cnt[A][T], cb = ctl->cnt[B][T];
+    int valid = ca != 0 && cb != 0;   // B5 / B10
     if (valid) {
-        for (int a = 0; a < 3; ++a) {
-            ctl->cgA[a] = __dmul_rn(__ddiv_rn((double)ctl->sum[A][a], (double)ca), 1.0 / 65536.0);
-            ctl->cgB[a] = __dmul_rn(__ddiv_rn((double)ctl->sum[B][a], (double)cb), 1.0 / 65536.0);
-        }
+        const int own[2] = {A, B};
+        for (int side = 0; side < 2; ++side)
+            for (int a = 0; a < 3; ++a) {
+                const int o = own[side];
+                const double ctyp = __dmul_rn(__ddiv_rn((double)ctl->sum[o][T][a], (double)ctl->cnt[o][T]), 1.0 / 65536.0);
+                double cg = ctyp;
+                if (typed) {   // Cg' = alpha Cg_alltypes + (1 - alpha) Cg_type
+                    long long sa = 0;
+                    unsigned long long na = 0;
+                    for (int t = 0; t < kBalTypes; ++t) { sa += ctl->sum[o][t][a]; na += ctl->cnt[o][t]; }
+                    const double call = __dmul_rn(__ddiv_rn((double)sa, (double)na), 1.0 / 65536.0);
+                    cg = __dadd_rn(__dmul_rn(alpha, call), __dmul_rn(__dsub_rn(1.0, alpha), ctyp));
+                }
+                (side == 0 ? ctl->cgA : ctl->cgB)[a] = cg;
+            }
         if (ctl->cgA[0] == ctl->cgB[0] && ctl->cgA[1] == ctl->cgB[1] && ctl->cgA[2] == ctl->cgB[2]) valid = 0;
     }
     ctl->valid = valid;
@@ -95,8 +112,9 @@ __device__ __forceinline__ int32_t balance_hash(const float4 &p, const double *o
 }
 
 __global__ void __launch_bounds__(256)
-bal_hash_kernel(int64_t n, const float4 *__restrict__ posm, const int32_t *__restrict__ owner, BalCtl *ctl,
-                int A, int B, int hmax, int32_t *__restrict__ bal_hash)
+bal_hash_kernel(int64_t n, const float4 *__restrict__ posm, const int32_t *__restrict__ owner,
+                const int32_t *__restrict__ ptype, BalCtl *ctl, int A, int B, int T, int hmax,
+                int32_t *__restrict__ bal_hash)
 {
     __shared__ uint32_t s_hist[2][kBalBins];
     for (int i = threadIdx.x; i < 2 * kBalBins; i += blockDim.x) (&s_hist[0][0])[i] = 0;
@@ -106,6 +124,7 @@ bal_hash_kernel(int64_t n, const float4 *__restrict__ posm, const int32_t *__res
              i += (int64_t)gridDim.x * blockDim.x) {
             const int o = owner[i];
             if (o != A && o != B) continue;
+            if (ptype && ptype[i] != T) continue;
             const float4 p = posm[i];
             const int side = o == A ? 0 : 1;
             const int32_t hv = side == 0 ? balance_hash(p, ctl->cgA, ctl->cgB, hmax)
@@ -143,16 +162,18 @@ __global__ void bal_pair_select_kernel(BalCtl *ctl, int hmax)
 
 // indicator arrays of the threshold ties (their exclusive scans rank the ties by id)
 __global__ void __launch_bounds__(256)
-bal_ties_kernel(int64_t n, const int32_t *__restrict__ owner, const int32_t *__restrict__ bal_hash,
-                const BalCtl *ctl, int A, int B, uint32_t *__restrict__ tieA, uint32_t *__restrict__ tieB)
+bal_ties_kernel(int64_t n, const int32_t *__restrict__ owner, const int32_t *__restrict__ ptype,
+                const int32_t *__restrict__ bal_hash, const BalCtl *ctl, int A, int B, int T,
+                uint32_t *__restrict__ tieA, uint32_t *__restrict__ tieB)
 {
     const int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
     if (i >= n) return;
     uint32_t a = 0, b = 0;
     if (ctl->valid) {
         const int o = owner[i];
-        if (o == A) a = (uint32_t)bal_hash[i] == ctl->thrA;
-        else if (o == B) b = (uint32_t)bal_hash[i] == ctl->thrB;
+        const bool mine = !ptype || ptype[i] == T;
+        if (mine && o == A) a = (uint32_t)bal_hash[i] == ctl->thrA;
+        else if (mine && o == B) b = (uint32_t)bal_hash[i] == ctl->thrB;
     }
     tieA[i] = a;
     tieB[i] = b;
@@ -160,8 +181,8 @@ bal_ties_kernel(int64_t n, const int32_t *__restrict__ owner, const int32_t *__r
 
 __global__ void __launch_bounds__(256)
 bal_swap_kernel(int64_t n, const float4 *__restrict__ posm, int32_t *__restrict__ owner,
-                const int32_t *__restrict__ bal_hash, BalCtl *ctl, int A, int B,
-                const uint32_t *__restrict__ rankA, const uint32_t *__restrict__ rankB)
+                const int32_t *__restrict__ ptype, const int32_t *__restrict__ bal_hash, BalCtl *ctl, int A,
+                int B, int T, const uint32_t *__restrict__ rankA, const uint32_t *__restrict__ rankB)
 {
     // D = (coordinates leaving A) - (coordinates leaving B): sum[A] -= D, sum[B] += D.  Exact
     // integer sums, so the order of the block and grid reductions does not matter.
@@ -173,7 +194,7 @@ bal_swap_kernel(int64_t n, const float4 *__restrict__ posm, int32_t *__restrict_
     long long f[3] = {0, 0, 0};
     if (i < n) {
         const int o = owner[i];
-        if (o == A || o == B) {
+        if ((o == A || o == B) && (!ptype || ptype[i] == T)) {
             const uint32_t hv = (uint32_t)bal_hash[i];
             const uint32_t thr = o == A ? ctl->thrA : ctl->thrB, quota = o == A ? ctl->quotaA : ctl->quotaB;
             const uint32_t rank = o == A ? rankA[i] : rankB[i];
@@ -195,8 +216,8 @@ bal_swap_kernel(int64_t n, const float4 *__restrict__ posm, int32_t *__restrict_
     __syncthreads();
     if (threadIdx.x < 3 && s_d[threadIdx.x]) {
         const long long d = s_d[threadIdx.x];
-        atomicAdd(reinterpret_cast<unsigned long long *>(&ctl->sum[A][threadIdx.x]), (unsigned long long)(-d));
-        atomicAdd(reinterpret_cast<unsigned long long *>(&ctl->sum[B][threadIdx.x]), (unsigned long long)d);
+        atomicAdd(reinterpret_cast<unsigned long long *>(&ctl->sum[A][T][threadIdx.x]), (unsigned long long)(-d));
+        atomicAdd(reinterpret_cast<unsigned long long *>(&ctl->sum[B][T][threadIdx.x]), (unsigned long long)d);
     }
 }
 
@@ -205,37 +226,41 @@ __global__ void bal_finish_kernel(const BalCtl *ctl, unsigned long long *swapped
     if (swapped_out) *swapped_out = ctl->swapped;
 }
 
-int launch_balance(sph_ctx *c, int64_t n, const float *posm, int32_t *owner, int hmax, int32_t *bal_hash,
-                   unsigned long long *swapped)
+int launch_balance(sph_ctx *c, int64_t n, const float *posm, int32_t *owner, const int32_t *ptype, int n_types,
+                   double alpha, int hmax, int32_t *bal_hash, unsigned long long *swapped)
 {
+    // ptype == NULL: single particle type, section III.A (plain Cg); else section III.B: the pair
+    // sweep per type with the biased Cg' of PAPER.md:56
     BalCtl *ctl = reinterpret_cast<BalCtl *>(c->bal);
     const float4 *p4 = reinterpret_cast<const float4 *>(posm);
     int32_t *bh = bal_hash ? bal_hash : reinterpret_cast<int32_t *>(c->s_hash);
     uint32_t *tieA = c->alt_keys, *tieB = c->alt_vals, *rankA = c->s_sorted_hash, *rankB = c->s_perm;
     SPH_CUDA_TRY(c, cudaMemsetAsync(ctl, 0, sizeof(BalCtl), c->stream));
     if (bal_hash) SPH_CUDA_TRY(c, cudaMemsetAsync(bal_hash, 0, sizeof(int32_t) * (size_t)n, c->stream));
-    const int G = c->params.n_owners;
+    const int G = c->params.n_owners, NT = ptype ? n_types : 1, typed = ptype != nullptr;
     if (n > 0 && G > 1) {
         const int blocks = (int)min((int64_t)c->num_sms * 8, (n + 255) / 256);
-        bal_sums_kernel<<<blocks, 256, 0, c->stream>>>(n, p4, owner, ctl);
+        bal_sums_kernel<<<blocks, 256, 0, c->stream>>>(n, p4, owner, ptype, ctl);
         SPH_CHECK_LAUNCH(c);
-        for (int A = 0; A < G; ++A)
-            for (int B = A + 1; B < G; ++B) {
-                bal_pair_begin_kernel<<<1, 256, 0, c->stream>>>(ctl, A, B);
-                SPH_CHECK_LAUNCH(c);
-                bal_hash_kernel<<<blocks, 256, 0, c->stream>>>(n, p4, owner, ctl, A, B, hmax, bh);
-                SPH_CHECK_LAUNCH(c);
-                bal_pair_select_kernel<<<1, 32, 0, c->stream>>>(ctl, hmax);
-                SPH_CHECK_LAUNCH(c);
-                bal_ties_kernel<<<div_up(n, 256), 256, 0, c->stream>>>(n, owner, bh, ctl, A, B, tieA, tieB);
-                SPH_CHECK_LAUNCH(c);
-                int rc = launch_scan_exclusive(c, n, tieA, rankA, nullptr);
-                if (rc != SPH_OK) return rc;
-                rc = launch_scan_exclusive(c, n, tieB, rankB, nullptr);
-                if (rc != SPH_OK) return rc;
-                bal_swap_kernel<<<div_up(n, 256), 256, 0, c->stream>>>(n, p4, owner, bh, ctl, A, B, rankA, rankB);
-                SPH_CHECK_LAUNCH(c);
-            }
+        for (int T = 0; T < NT; ++T)
+            for (int A = 0; A < G; ++A)
+                for (int B = A + 1; B < G; ++B) {
+                    bal_pair_begin_kernel<<<1, 256, 0, c->stream>>>(ctl, A, B, T, typed, alpha);
+                    SPH_CHECK_LAUNCH(c);
+                    bal_hash_kernel<<<blocks, 256, 0, c->stream>>>(n, p4, owner, ptype, ctl, A, B, T, hmax, bh);
+                    SPH_CHECK_LAUNCH(c);
+                    bal_pair_select_kernel<<<1, 32, 0, c->stream>>>(ctl, hmax);
+                    SPH_CHECK_LAUNCH(c);
+                    bal_ties_kernel<<<div_up(n, 256), 256, 0, c->stream>>>(n, owner, ptype, bh, ctl, A, B, T, tieA, tieB);
+                    SPH_CHECK_LAUNCH(c);
+                    int rc = launch_scan_exclusive(c, n, tieA, rankA, nullptr);
+                    if (rc != SPH_OK) return rc;
+                    rc = launch_scan_exclusive(c, n, tieB, rankB, nullptr);
+                    if (rc != SPH_OK) return rc;
+                    bal_swap_kernel<<<div_up(n, 256), 256, 0, c->stream>>>(n, p4, owner, ptype, bh, ctl, A, B, T,
+                                                                          rankA, rankB);
+                    SPH_CHECK_LAUNCH(c);
+                }
     }
     bal_finish_kernel<<<1, 1, 0, c->stream>>>(ctl, swapped);
     SPH_CHECK_LAUNCH(c);

@@ -210,7 +210,16 @@ int sph_balance(sph_ctx *c, int64_t n, const float *posm, int32_t *owner, int32_
                 unsigned long long *swapped)
 {
     if (!n_ok(c, n) || !posm || !owner || hmax < 1 || hmax > 1023) return SPH_EINVAL;
-    return launch_balance(c, n, posm, owner, hmax, bal_hash, swapped);
+    return launch_balance(c, n, posm, owner, nullptr, 1, 0.0, hmax, bal_hash, swapped);
+}
+
+int sph_balance_types(sph_ctx *c, int64_t n, const float *posm, int32_t *owner, const int32_t *ptype,
+                      int32_t n_types, double alpha, int32_t hmax, int32_t *bal_hash, unsigned long long *swapped)
+{
+    if (!n_ok(c, n) || !posm || !owner || !ptype || hmax < 1 || hmax > 1023 || n_types < 1 || n_types > 8 ||
+        !(alpha >= 0.0 && alpha <= 1.0))
+        return SPH_EINVAL;
+    return launch_balance(c, n, posm, owner, ptype, n_types, alpha, hmax, bal_hash, swapped);
 }
 
 int sph_cell_ranges(sph_ctx *c, int64_t n, const uint32_t *sorted_hash, uint32_t *cs, uint32_t *ce)

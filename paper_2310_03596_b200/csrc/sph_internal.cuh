@@ -129,8 +129,8 @@ int launch_partition_by_label(sph_ctx *c, int64_t m, const uint32_t *ids, const 
                               uint32_t *offsets, uint32_t *dest /* [m] scatter map */);
 int launch_scatter_records(sph_ctx *c, int64_t m, const uint32_t *ids, const uint32_t *dest,
                            const sph_state *in, const sph_state *out, uint32_t *packed_ids);
-int launch_balance(sph_ctx *c, int64_t n, const float *posm, int32_t *owner, int hmax, int32_t *bal_hash,
-                   unsigned long long *swapped);
+int launch_balance(sph_ctx *c, int64_t n, const float *posm, int32_t *owner, const int32_t *ptype, int n_types,
+                   double alpha, int hmax, int32_t *bal_hash, unsigned long long *swapped);
 size_t balance_scratch_bytes();
 int launch_scan_exclusive(sph_ctx *c, int64_t n, const uint32_t *in, uint32_t *out,
                           uint32_t *total /* dev scalar */);

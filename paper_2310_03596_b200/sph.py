@@ -29,7 +29,7 @@ FLAG_INTERACT_DIRECT = 1
 EXPORTS = (
     "sph_create", "sph_destroy", "sph_hash", "sph_sort", "sph_reorder", "sph_cell_ranges",
     "sph_comm_hash", "sph_interact", "sph_integrate", "sph_step", "sph_step_host", "sph_pack_boundary",
-    "sph_interact_split", "sph_balance", "sph_enable_timing", "sph_get_timing", "sph_launch_count", "sph_strerror",
+    "sph_interact_split", "sph_balance", "sph_balance_types", "sph_enable_timing", "sph_get_timing", "sph_launch_count", "sph_strerror",
     "sph_last_cuda_error",
 )
 
@@ -75,6 +75,7 @@ def load_library() -> C.CDLL:
     lib.sph_step.argtypes = [vp, i64, f32, sp] + [vp] * 11 + [C.POINTER(vp * 6), vp]
     lib.sph_step_host.argtypes = [vp, i64, f32, i32, sp, vp, vp, vp]
     lib.sph_balance.argtypes = [vp, i64, vp, vp, i32, vp, vp]
+    lib.sph_balance_types.argtypes = [vp, i64, vp, vp, vp, i32, C.c_double, i32, vp, vp]
     lib.sph_pack_boundary.argtypes = [vp, i64, i64, sp, vp, vp, vp, sp]
     lib.sph_enable_timing.argtypes = [vp, i32]
     lib.sph_get_timing.argtypes = [vp, C.POINTER(f32 * 8)]
@@ -358,6 +359,17 @@ class Context:
                                        bh.data_ptr(), sw.data_ptr()), "sph_balance")
         return bh[:n], sw
 
+    def sph_balance_types(self, posm: torch.Tensor, owner: torch.Tensor, ptype: torch.Tensor, n_types: int,
+                          alpha: float = 0.1, hmax: int = 1000):
+        """Balancing sweep per particle type with the biased Cg' of PAPER.md:56 (NEXT-4)."""
+        n = int(posm.shape[0])
+        bh = self._i32(max(n, 1))
+        sw = torch.zeros(1, dtype=torch.int64, device=self.device)
+        self._chk(self.lib.sph_balance_types(self.handle, n, posm.data_ptr(), owner.data_ptr(), ptype.data_ptr(),
+                                             int(n_types), float(alpha), int(hmax), bh.data_ptr(), sw.data_ptr()),
+                  "sph_balance_types")
+        return bh[:n], sw
+
     def sph_pack_boundary(self, state: State, boundary_ids: torch.Tensor, m: int):
         """Per-owner send buffers (NEXT-1): returns (owner_offsets [n_owners + 1], packed_ids [m],
         packed State of length m).  m is the host value of boundary_count."""
@@ -397,3 +409,4 @@ def sph_step(ctx, *a, **k): return ctx.sph_step(*a, **k)
 def sph_step_host(ctx, *a, **k): return ctx.sph_step_host(*a, **k)
 def sph_pack_boundary(ctx, *a, **k): return ctx.sph_pack_boundary(*a, **k)
 def sph_balance(ctx, *a, **k): return ctx.sph_balance(*a, **k)
+def sph_balance_types(ctx, *a, **k): return ctx.sph_balance_types(*a, **k)

@@ -351,3 +351,28 @@ def test_balance_sweep_matches_oracle_bit_exact(sph, oracle, make, g):
         np.testing.assert_array_equal(own_gpu.cpu().numpy(), own_ref, err_msg=f"owner sweep {sweep}")
         np.testing.assert_array_equal(np.bincount(own_ref, minlength=g), np.bincount(w.owner, minlength=g))
     ctx.close()
+
+
+@pytest.mark.parametrize("g,nt,alpha", [(3, 2, 0.1), (5, 3, 0.1), (4, 2, 1.0), (4, 1, 0.0)])
+def test_balance_types_matches_oracle_bit_exact(sph, oracle, g, nt, alpha):
+    """sph_balance_types (Cg' = alpha Cg_all + (1 - alpha) Cg_type) against
+    oracle.balance_types, bit-exact over two sweeps; every (owner, type) count is kept."""
+    w = wl.lattice_block(26, 22, 20, 0.1, 31 + g, owners=("random", g))
+    rng = np.random.default_rng(100 + g)
+    ptype = rng.integers(0, nt, w.n).astype(np.int32)
+    ctx = sph.Context.for_workload(w)
+    posm = torch.from_numpy(w.posm).cuda()
+    pt = torch.from_numpy(ptype).cuda()
+    own_gpu = torch.from_numpy(w.owner.copy()).cuda()
+    own_ref = w.owner.copy()
+    for sweep in range(2):
+        bh, sw = ctx.sph_balance_types(posm, own_gpu, pt, nt, alpha)
+        torch.cuda.synchronize()
+        own_ref, k, bh_ref = oracle.balance_types(w.posm, own_ref, ptype, g, nt, alpha=alpha)
+        assert int(sw.cpu()[0]) == k and k > 0
+        np.testing.assert_array_equal(bh.cpu().numpy(), bh_ref)
+        np.testing.assert_array_equal(own_gpu.cpu().numpy(), own_ref)
+    for t in range(nt):
+        np.testing.assert_array_equal(np.bincount(own_ref[ptype == t], minlength=g),
+                                      np.bincount(w.owner[ptype == t], minlength=g))
+    ctx.close()
