@@ -204,6 +204,22 @@ def test_error_codes(sph):
     ctx = sph.Context([0, 0, 0], [4, 4, 4], 1.3, max_n=8)
     with pytest.raises(sph.SphError):
         ctx.sph_hash(torch.zeros((9, 4), device="cuda"))       # n > max_n
+    # the NEXT entry points reject bad arguments the same way
+    posm = torch.zeros((8, 4), device="cuda")
+    own = torch.zeros(8, dtype=torch.int32, device="cuda")
+    with pytest.raises(sph.SphError):
+        ctx.sph_balance(posm, own, hmax=0)
+    with pytest.raises(sph.SphError):
+        ctx.sph_balance(posm, own, hmax=2000)
+    with pytest.raises(sph.SphError):
+        ctx.sph_balance_types(posm, own, own, n_types=9)
+    with pytest.raises(sph.SphError):
+        ctx.sph_balance_types(posm, own, own, n_types=2, alpha=1.5)
+    st = sph.State.empty(8)
+    with pytest.raises(sph.SphError):
+        ctx.sph_pack_boundary(st, own, 9)                      # m > n
+    with pytest.raises(sph.SphError):
+        ctx.sph_interact_split(st, own, own, own, 3)           # which must be 1 or 2
     ctx.close()
 
 
