@@ -145,3 +145,10 @@ def test_config2_full_size(sph, oracle):
 def test_config4_full_size(sph, oracle):
     """configs[4], 64 M particles (the maximum size): 22-bit keys, 7 813 onesweep tiles."""
     _fullsize_case(sph, oracle, 4, steps_before=1, expect_boundary=(0.999, 1.0))
+
+
+@pytest.mark.skipif(os.environ.get("SPH_SKIP_22M") == "1", reason="SPH_SKIP_22M=1")
+def test_config3_full_size(sph, oracle):
+    """configs[3], the irregular geometry as stated (22.0 M particles: plate + 8 cylinders, long
+    runs of empty buckets, 16 owners by recursive coordinate bisection)."""
+    _fullsize_case(sph, oracle, 3, steps_before=1, expect_boundary=(0.05, 0.35))
