@@ -392,3 +392,28 @@ def test_balance_types_matches_oracle_bit_exact(sph, oracle, g, nt, alpha):
         np.testing.assert_array_equal(np.bincount(own_ref[ptype == t], minlength=g),
                                       np.bincount(w.owner[ptype == t], minlength=g))
     ctx.close()
+
+
+def test_long_run_then_lockstep(sph, oracle):
+    """300 steps of the benchmark's configuration on a scaled configs[1] (state re-hashed and
+    re-sorted every step), then one lock-step comparison with the oracle from the GPU's state:
+    accumulated drift must not break any stage (particles have moved across bucket faces by then)."""
+    w = wl.config(1, side=33)
+    ctx = sph.Context.for_workload(w)
+    state = sph.State.from_numpy(w.posm, w.velr, w.sig, w.owner)
+    for _ in range(300):
+        ctx.sph_step(state, 10 * w.dt)                 # larger dt: particles really travel
+    torch.cuda.synchronize()
+    posm, velr = state.posm.cpu().numpy(), state.velr.cpu().numpy()
+    sig, owner = state.sig.cpu().numpy(), state.owner.cpu().numpy()
+    assert np.isfinite(posm).all() and np.isfinite(velr).all() and np.isfinite(sig).all()
+    moved = np.abs(posm[:, :3] - w.posm[:, :3]).max()
+    assert moved > 1e-3, moved
+    ref = oracle.step(posm, velr, sig, owner, w.origin, w.dims, w.h, w.K, w.G, w.n_owners, w.dt)
+    out = ctx.alloc_outputs(w.n)
+    ctx.sph_step(state, w.dt, out)
+    torch.cuda.synchronize()
+    parity.compare_integers(out, ref, w.n)
+    parity.compare_rates(out, ref.rates)
+    parity.compare_state(state, ref)
+    ctx.close()
