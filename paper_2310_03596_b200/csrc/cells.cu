@@ -1,13 +1,13 @@
 // Stage 2c: cell start/end tables (BASELINE.json north_star; reading S7).
 // cell_start[c] = #{k : sorted_hash[k] < c},  cell_end[c] = #{k : sorted_hash[k] <= c}.
-// One thread per 4 sorted particles (one 128-bit load) marks the run boundaries; runs of EMPTY buckets between two
+// One thread per 8 sorted particles (two 128-bit loads) marks the run boundaries; runs of EMPTY buckets between two
 // occupied ones (long in config 3's clipped geometry) are filled by the whole warp, not by one
 // thread.  Traffic: 4 B read per particle + 8 B written per bucket.
 #include "sph_internal.cuh"
 
 namespace sphb {
 
-constexpr int kCellItems = 4;  // sorted positions per thread (one 128-bit load)
+constexpr int kCellItems = 8;  // sorted positions per thread (two 128-bit loads in flight)
 
 // boundary between sorted positions k-1 (hash hp) and k (hash hc): closes bucket hp, opens hc;
 // the empty buckets in between get start == end == k.  Returns the gap range for the caller.
@@ -20,7 +20,7 @@ __device__ __forceinline__ void mark_boundary(int64_t k, int64_t n, int64_t hp, 
     if (k > 0) ce[hp] = (uint32_t)k;
     const int64_t l = hp + 1, h = hc - 1;
     if (h - l + 1 > 4) {        // at most one long gap is kept per thread; earlier ones are
-        if (hi >= lo)           // written inline (rare: two long gaps inside 4 positions)
+        if (hi >= lo)           // written inline (rare: two long gaps inside 8 positions)
             for (int64_t c = lo; c <= hi; ++c) { cs[c] = fill; ce[c] = fill; }
         lo = l; hi = h; fill = (uint32_t)k;
     } else {
@@ -32,13 +32,16 @@ __global__ void __launch_bounds__(256)
 cell_ranges_kernel(int64_t n, const uint32_t *__restrict__ sorted_hash, uint32_t *__restrict__ cs,
                    uint32_t *__restrict__ ce, uint32_t n_cells)
 {
-    // thread t owns the boundaries k = 4t .. 4t+3 (k == n closes the table)
+    // thread t owns the boundaries k = 8t .. 8t+7 (k == n closes the table)
     const int64_t k0 = ((int64_t)blockIdx.x * blockDim.x + threadIdx.x) * kCellItems;
     const int lane = threadIdx.x & 31;
     int64_t hcur[kCellItems];
     if (k0 + kCellItems <= n && (reinterpret_cast<uintptr_t>(sorted_hash) & 15) == 0) {
-        const uint4 v = __ldcs(reinterpret_cast<const uint4 *>(sorted_hash + k0));
-        hcur[0] = v.x; hcur[1] = v.y; hcur[2] = v.z; hcur[3] = v.w;
+#pragma unroll
+        for (int q = 0; q < kCellItems / 4; ++q) {
+            const uint4 v = __ldcs(reinterpret_cast<const uint4 *>(sorted_hash + k0) + q);
+            hcur[4 * q] = v.x; hcur[4 * q + 1] = v.y; hcur[4 * q + 2] = v.z; hcur[4 * q + 3] = v.w;
+        }
     } else {
 #pragma unroll
         for (int j = 0; j < kCellItems; ++j)
