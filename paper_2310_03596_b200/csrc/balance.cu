@@ -138,26 +138,52 @@ bal_hash_kernel(int64_t n, const float4 *__restrict__ posm, const int32_t *__res
         if ((&s_hist[0][0])[i]) atomicAdd(&ctl->hist[0][0] + i, (&s_hist[0][0])[i]);
 }
 
-// one thread: n = min(nA, nB); per side the threshold hash and the number of its ties that move
-__global__ void bal_pair_select_kernel(BalCtl *ctl, int hmax)
+// one block of kBalBins threads: n = min(nA, nB); per side the threshold hash and the number of
+// its ties that move.  Thread j owns hash value h = kBalBins - 1 - j, so an inclusive scan over j is
+// the count of particles with a hash >= h.
+__global__ void __launch_bounds__(kBalBins) bal_pair_select_kernel(BalCtl *ctl, int hmax)
 {
-    if (threadIdx.x != 0 || !ctl->valid) return;
-    unsigned long long tot[2] = {0, 0};
-    for (int s = 0; s < 2; ++s)
-        for (int h = 1; h <= hmax; ++h) tot[s] += ctl->hist[s][h];
-    const unsigned long long m = tot[0] < tot[1] ? tot[0] : tot[1];
-    if (m == 0) { ctl->valid = 0; return; }
+    __shared__ unsigned int s_warp[2][kBalBins / 32];
+    __shared__ unsigned int s_tot[2];
+    if (!ctl->valid) return;   // uniform
+    const int j = threadIdx.x, lane = j & 31, w = j >> 5;
+    const int h = kBalBins - 1 - j;
+    unsigned int cnt[2], inc[2];
+#pragma unroll
     for (int s = 0; s < 2; ++s) {
-        unsigned long long above = 0;
-        int h = hmax;
-        for (; h >= 1; --h) {
-            if (above + ctl->hist[s][h] >= m) break;
-            above += ctl->hist[s][h];
+        cnt[s] = (h >= 1 && h <= hmax) ? ctl->hist[s][h] : 0u;
+        unsigned int v = cnt[s];
+#pragma unroll
+        for (int o = 1; o < 32; o <<= 1) {
+            const unsigned int x = __shfl_up_sync(0xffffffffu, v, o);
+            if (lane >= o) v += x;
         }
-        (s == 0 ? ctl->thrA : ctl->thrB) = (uint32_t)h;
-        (s == 0 ? ctl->quotaA : ctl->quotaB) = (uint32_t)(m - above);
+        inc[s] = v;
+        if (lane == 31) s_warp[s][w] = v;
     }
-    ctl->swapped += m;
+    __syncthreads();
+#pragma unroll
+    for (int s = 0; s < 2; ++s) {
+        unsigned int add = 0;
+        for (int i = 0; i < w; ++i) add += s_warp[s][i];
+        inc[s] += add;                       // particles of side s with a hash >= h
+        if (j == kBalBins - 1) s_tot[s] = inc[s];
+    }
+    __syncthreads();
+    const unsigned int m = min(s_tot[0], s_tot[1]);
+    if (m == 0) {
+        if (j == 0) ctl->valid = 0;
+        return;
+    }
+#pragma unroll
+    for (int s = 0; s < 2; ++s) {
+        const unsigned int above = inc[s] - cnt[s];            // hash > h
+        if (above < m && inc[s] >= m && cnt[s] > 0) {          // h is the threshold of side s
+            (s == 0 ? ctl->thrA : ctl->thrB) = (uint32_t)h;
+            (s == 0 ? ctl->quotaA : ctl->quotaB) = m - above;
+        }
+    }
+    if (j == 0) ctl->swapped += m;
 }
 
 // indicator arrays of the threshold ties (their exclusive scans rank the ties by id)
@@ -249,7 +275,7 @@ int launch_balance(sph_ctx *c, int64_t n, const float *posm, int32_t *owner, con
                     SPH_CHECK_LAUNCH(c);
                     bal_hash_kernel<<<blocks, 256, 0, c->stream>>>(n, p4, owner, ptype, ctl, A, B, T, hmax, bh);
                     SPH_CHECK_LAUNCH(c);
-                    bal_pair_select_kernel<<<1, 32, 0, c->stream>>>(ctl, hmax);
+                    bal_pair_select_kernel<<<1, kBalBins, 0, c->stream>>>(ctl, hmax);
                     SPH_CHECK_LAUNCH(c);
                     bal_ties_kernel<<<div_up(n, 256), 256, 0, c->stream>>>(n, owner, ptype, bh, ctl, A, B, T, tieA, tieB);
                     SPH_CHECK_LAUNCH(c);
