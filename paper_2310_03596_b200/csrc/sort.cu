@@ -419,10 +419,23 @@ scan_exclusive_kernel(int64_t n, const uint32_t *__restrict__ in, uint32_t *__re
     const int64_t base = (int64_t)tile * kScanTile + (int64_t)tid * kScanItems;
     uint32_t v[kScanItems];
     uint32_t sum = 0;
+    static_assert(kScanItems % 4 == 0, "128-bit loads and stores");
+    const bool vec = base + kScanItems <= n &&
+                     ((reinterpret_cast<uintptr_t>(in) | reinterpret_cast<uintptr_t>(out)) & 15) == 0;
+    if (vec) {
 #pragma unroll
-    for (int i = 0; i < kScanItems; ++i) {
-        v[i] = (base + i < n) ? in[base + i] : 0u;
-        sum += v[i];
+        for (int q = 0; q < kScanItems / 4; ++q) {
+            const uint4 x = __ldcs(reinterpret_cast<const uint4 *>(in + base) + q);
+            v[4 * q] = x.x; v[4 * q + 1] = x.y; v[4 * q + 2] = x.z; v[4 * q + 3] = x.w;
+        }
+#pragma unroll
+        for (int i = 0; i < kScanItems; ++i) sum += v[i];
+    } else {
+#pragma unroll
+        for (int i = 0; i < kScanItems; ++i) {
+            v[i] = (base + i < n) ? in[base + i] : 0u;
+            sum += v[i];
+        }
     }
     uint32_t inc = sum;
 #pragma unroll
@@ -468,10 +481,19 @@ scan_exclusive_kernel(int64_t n, const uint32_t *__restrict__ in, uint32_t *__re
     }
     __syncthreads();
     uint32_t run = s_excl + add + (inc - sum);
+    if (vec) {
+        uint32_t o[kScanItems];
 #pragma unroll
-    for (int i = 0; i < kScanItems; ++i) {
-        if (base + i < n) out[base + i] = run;
-        run += v[i];
+        for (int i = 0; i < kScanItems; ++i) { o[i] = run; run += v[i]; }
+#pragma unroll
+        for (int q = 0; q < kScanItems / 4; ++q)
+            __stcs(reinterpret_cast<uint4 *>(out + base) + q, make_uint4(o[4 * q], o[4 * q + 1], o[4 * q + 2], o[4 * q + 3]));
+    } else {
+#pragma unroll
+        for (int i = 0; i < kScanItems; ++i) {
+            if (base + i < n) out[base + i] = run;
+            run += v[i];
+        }
     }
 }
 
