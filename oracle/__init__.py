@@ -51,7 +51,7 @@ def _load():
                                  vp, vp, vp, vp, vp]
     lib.orc_interact.restype = None
     lib.orc_interact_split.argtypes = [i64, vp, vp, vp, vp, vp, vp, vp, f32, f32, f32, vp, C.c_int,
-                                       vp, vp, vp, vp, vp]
+                                       i64, vp, vp, vp, vp, vp, vp]
     lib.orc_interact_split.restype = None
     lib.orc_integrate.argtypes = [i64, f64, vp, vp, vp, vp, vp, vp, vp, vp, vp]
     lib.orc_integrate.restype = None
@@ -224,9 +224,11 @@ def interact(posm, velr, sig, sorted_hash, dims, cell_start, cell_end, h, K, G, 
     return Rates(drho, L, acc, dsig, int(pc.value))
 
 
-def interact_split(posm, velr, sig, sorted_hash, dims, cell_start, cell_end, h, K, G, owner, which) -> Rates:
+def interact_split(posm, velr, sig, sorted_hash, dims, cell_start, cell_end, h, K, G, owner, which,
+                   idx=None) -> Rates:
     """Step e alone (which = 1: same-owner neighbours) or step f alone (which = 2: other owners);
-    sph_oracle.c orc_interact_split.  All arrays in sorted order."""
+    sph_oracle.c orc_interact_split.  All arrays in sorted order; idx = sorted
+    positions to compute (None = all)."""
     posm = _c(posm, np.float32)
     velr = _c(velr, np.float32)
     sig = _c(sig, np.float32)
@@ -236,14 +238,21 @@ def interact_split(posm, velr, sig, sorted_hash, dims, cell_start, cell_end, h, 
     dims = _c(dims, np.int32)
     cell_start = _c(cell_start, np.uint32)
     cell_end = _c(cell_end, np.uint32)
-    drho = np.zeros(n, np.float64)
-    L = np.zeros((n, 3, 3), np.float64)
-    acc = np.zeros((n, 3), np.float64)
-    dsig = np.zeros((n, 6), np.float64)
+    if idx is not None:
+        idx = _c(idx, np.int64)
+        m = idx.shape[0]
+    else:
+        m = n
+    drho = np.zeros(m, np.float64)
+    L = np.zeros((m, 3, 3), np.float64)
+    acc = np.zeros((m, 3), np.float64)
+    dsig = np.zeros((m, 6), np.float64)
     pc = C.c_int64(0)
     _load().orc_interact_split(n, _p(posm), _p(velr), _p(sig), _p(sorted_hash), _p(dims), _p(cell_start),
                                _p(cell_end), np.float32(h), np.float32(K), np.float32(G), _p(owner),
-                               int(which), _p(drho), _p(L), _p(acc), _p(dsig), C.byref(pc))
+                               int(which), m if idx is not None else 0,
+                               _p(idx) if idx is not None else None,
+                               _p(drho), _p(L), _p(acc), _p(dsig), C.byref(pc))
     return Rates(drho, L, acc, dsig, int(pc.value))
 
 

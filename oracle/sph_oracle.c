@@ -381,15 +381,16 @@ void orc_interact(int64_t n, const float *posm, const float *velr, const float *
                       n_idx, idx, NULL, 0, drho, L, acc, dsig, pair_count);
 }
 
-/* NEXT-3: steps e (which = 1) and f (which = 2) as separate passes; owner is in sorted order. */
+/* NEXT-3: steps e (which = 1) and f (which = 2) as separate passes; owner is in sorted order.
+ * idx != NULL: only the n_idx sorted positions idx[] are computed (sampled parity at full size). */
 void orc_interact_split(int64_t n, const float *posm, const float *velr, const float *sig,
                         const uint32_t *sorted_hash, const int32_t *dims, const uint32_t *cell_start,
                         const uint32_t *cell_end, float h_f32, float K_f32, float G_f32,
-                        const int32_t *owner, int which,
+                        const int32_t *owner, int which, int64_t n_idx, const int64_t *idx,
                         double *drho, double *L, double *acc, double *dsig, int64_t *pair_count)
 {
     orc_interact_impl(n, posm, velr, sig, sorted_hash, dims, cell_start, cell_end, h_f32, K_f32, G_f32,
-                      0, NULL, owner, which, drho, L, acc, dsig, pair_count);
+                      n_idx, idx, owner, which, drho, L, acc, dsig, pair_count);
 }
 
 /* ------------------------------------------------------------------------------------------

@@ -512,20 +512,43 @@ def test_split_passes_sum_to_the_single_pass_and_match_bruteforce():
     for name in ("drho", "acc", "dsig", "L"):
         a, b, c = getattr(e, name), getattr(f, name), getattr(full, name)
         assert np.max(np.abs(a + b - c)) <= 1e-13 * max(np.max(np.abs(c)), 1e-300), name
-    # dense evaluation of the other-owner pairs only (momentum part: sigma_i term included per pair)
+    # dense O(N^2) evaluation by distance only, restricted to same-owner pairs (pass e) and to
+    # other-owner pairs (pass f): EVERY output of both loops (drho and L of loop 1, acc of loop 2,
+    # dsig from the dense L), so that a swapped owner filter in either loop fails here
     x = sp[:, :3].astype(np.float64); m = sp[:, 3].astype(np.float64)
     v = sv[:, :3].astype(np.float64); rho = sv[:, 3].astype(np.float64)
+    sg = ss.astype(np.float64)
+    S = np.empty((w.n, 3, 3))
+    S[:, 0, 0], S[:, 1, 1], S[:, 2, 2] = sg[0], sg[1], sg[2]
+    S[:, 0, 1] = S[:, 1, 0] = sg[3]; S[:, 0, 2] = S[:, 2, 0] = sg[4]; S[:, 1, 2] = S[:, 2, 1] = sg[5]
+    Sr = S / (rho ** 2)[:, None, None]
     h = float(w.h)
     xij = x[:, None, :] - x[None, :, :]
     rr = np.sqrt((xij ** 2).sum(-1))
-    nb = (rr < 2 * h) & ~np.eye(w.n, dtype=bool) & (so[:, None] != so[None, :])
+    inside = (rr < 2 * h) & ~np.eye(w.n, dtype=bool)
     alpha = 21.0 / (16.0 * np.pi * h ** 3)
-    Fm = np.where(nb, -(5.0 * alpha / h ** 2) * (1 - rr / (2 * h)) ** 3, 0.0)
-    gW = Fm[..., None] * xij
     vij = v[:, None, :] - v[None, :, :]
-    drho = (m[None, :] * (vij * gW).sum(-1)).sum(1)
-    np.testing.assert_allclose(f.drho, drho, rtol=0, atol=1e-12 * np.max(np.abs(drho)))
-    assert f.pair_count == int(nb.sum())
+    for res, sel in ((e, so[:, None] == so[None, :]), (f, so[:, None] != so[None, :])):
+        nb = inside & sel
+        Fm = np.where(nb, -(5.0 * alpha / h ** 2) * (1 - rr / (2 * h)) ** 3, 0.0)
+        gW = Fm[..., None] * xij                                     # [i, j, b]
+        drho = (m[None, :] * (vij * gW).sum(-1)).sum(1)
+        Ld = np.einsum("j,ija,ijb->iab", m / rho, -vij, gW)          # L[a][b] = sum V_j (v_j - v_i)_a gW_b
+        accd = np.einsum("j,ijab,ijb->ia", m, Sr[:, None] + Sr[None, :], gW)
+        D = 0.5 * (Ld + Ld.transpose(0, 2, 1)); Om = 0.5 * (Ld - Ld.transpose(0, 2, 1))
+        trD = np.trace(D, axis1=1, axis2=2)
+        sd = (w.K * trD)[:, None, None] * np.eye(3) + 2 * w.G * (D - (trD / 3)[:, None, None] * np.eye(3)) \
+            + Om @ S - S @ Om
+        dsd = np.stack([sd[:, 0, 0], sd[:, 1, 1], sd[:, 2, 2], sd[:, 0, 1], sd[:, 0, 2], sd[:, 1, 2]], 1)
+        for name, ref in (("drho", drho), ("L", Ld), ("acc", accd), ("dsig", dsd)):
+            got = getattr(res, name)
+            assert np.max(np.abs(got - ref)) <= 1e-11 * np.max(np.abs(ref)), name
+        assert res.pair_count == int(nb.sum())
+    # the sampled form (idx) returns the same rows
+    pick = np.array([0, 7, w.n // 2, w.n - 1])
+    fs = orc.interact_split(*args, so, 2, idx=pick)
+    np.testing.assert_array_equal(fs.acc, f.acc[pick])
+    np.testing.assert_array_equal(fs.dsig, f.dsig[pick])
 
 
 # ----------------------------------------------------------------------------- NEXT-2: balancing
