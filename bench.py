@@ -5,7 +5,8 @@
 
 A "step" is one pass of the whole hot path (sph_step: hash -> onesweep sort -> reorder -> cell
 ranges -> comm hash + compaction -> interaction loops with the integration in their epilogue) over the particles of
-BASELINE.json configs[k] (default k = 1, the 1 M-particle block).  N > 1 (torchrun) runs N
+BASELINE.json configs[k] (default k = 4: 64 M particles, the largest single-GPU configuration, the one
+the roofline bars of BASELINE.json's north_star are about; k = 0..3 are parity-test sizes).  N > 1 (torchrun) runs N
 independent replicas (the one-GPU path does not shard; "weak" scaling).
 
 `value`     particles/s, inputs resident in HBM, CUDA-event time of the K steps (L2 flushed
@@ -231,21 +232,25 @@ def run_ours(args, rank, world, local_rank):
         sampler.start()
     launches0 = ctx.launch_count()
     evs = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(K)]
-    stage_ms = {}
+    stage_ms, stage_w = {}, 0
+    ctx.enable_timing(True)                             # resets the library's ring of stage events
     barrier()
     for it in range(K):
         flush.zero_()                                   # L2 flush, outside the timed interval
         evs[it][0].record()
         ctx.sph_step(state, w.dt)                       # pair_count = NULL: the count is optional (include/sph.h)
         evs[it][1].record()
-        if args.stage_timing:
+        if (it + 1) % sph.TIMING_SLOTS == 0 or it == K - 1:
+            # the stage events live in a ring of TIMING_SLOTS steps inside the library: drain it
+            # (one host sync per ring, between steps) so that EVERY timed step enters the average
+            m_ = (it % sph.TIMING_SLOTS) + 1
             for k_, v in ctx.get_timing().items():
-                stage_ms[k_] = stage_ms.get(k_, 0.0) + v / K
+                stage_ms[k_] = stage_ms.get(k_, 0.0) + v * m_
+            stage_w += m_
     barrier()
     launches = ctx.launch_count() - launches0
     total_ms = sum(a.elapsed_time(b) for a, b in evs)
-    if not args.stage_timing:                            # stage times of the last step only
-        stage_ms = ctx.get_timing()
+    stage_ms = {k_: v / stage_w for k_, v in stage_ms.items()}
     total_ms = max_over_ranks(total_ms, world, dev)
 
     # ---- NEXT-1 (not part of the step metric): per-owner send buffers of the last boundary list ----
@@ -408,12 +413,11 @@ def run_ours(args, rank, world, local_rank):
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
-    ap.add_argument("--steps", type=int, default=200)
+    ap.add_argument("--steps", type=int, default=20)
     ap.add_argument("--warmup", type=int, default=3)
-    ap.add_argument("--config", type=int, default=1, help="BASELINE.json configs[k]")
+    ap.add_argument("--config", type=int, default=4, help="BASELINE.json configs[k] (default: the 64 M-particle headline)")
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--flags", type=int, default=0, help="sph_params.flags (1 = direct interaction kernel)")
-    ap.add_argument("--stage-timing", action="store_true", help="average stage times over all steps (syncs each step)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--balance-sweeps", type=int, default=2, help="NEXT-2 report: balancing sweeps to time (0 = skip)")
     ap.add_argument("--cpu-sample", type=int, default=300000)

@@ -218,10 +218,11 @@ int sph_balance_types(sph_ctx *ctx, int64_t n, const float *posm, int32_t *owner
 int sph_step_host(sph_ctx *ctx, int64_t n, float dt, int32_t steps, const sph_state *host_state,
                   uint32_t *boundary_ids, uint32_t *boundary_count, unsigned long long *pair_count);
 
-/* Per-stage device time of the most recent sph_step, measured with CUDA events recorded on the
- * ctx's stream (enabled by sph_enable_timing(ctx, 1); adds no host sync to sph_step itself --
- * this call synchronises).  ms[0..7] = hash, sort, reorder, cell_ranges, comm_hash, interact,
- * integrate, total. */
+/* Per-stage device time of sph_step, measured with CUDA events recorded on the ctx's stream
+ * (enabled by sph_enable_timing(ctx, 1); adds no host sync to sph_step itself -- sph_get_timing
+ * synchronises).  ms[0..7] = hash, sort, reorder, cell_ranges, comm_hash, interact, integrate,
+ * total, each the AVERAGE over the steps enqueued since the last sph_get_timing / enable call (at
+ * most the 32 most recent: the events live in a ring).  SPH_EINVAL if no step was recorded. */
 int sph_enable_timing(sph_ctx *ctx, int32_t on);
 int sph_get_timing(sph_ctx *ctx, float ms[8]);
 

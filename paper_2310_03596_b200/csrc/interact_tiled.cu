@@ -601,9 +601,8 @@ int launch_interact_tiled(sph_ctx *c, int64_t n, const InteractIn &in, const uin
         SPH_CHECK_LAUNCH(c);
     }
     c->rec_fresh = false;
-    static bool attr_set = false;
     const int smem = (int)sizeof(TileSmem);
-    if (!attr_set) {
+    if (!c->attr_interact) {   // per device: once per ctx
         SPH_CUDA_TRY(c, cudaFuncSetAttribute(interact_tiled_kernel<true, kPassAll>,
                                              cudaFuncAttributeMaxDynamicSharedMemorySize, smem));
         SPH_CUDA_TRY(c, cudaFuncSetAttribute(interact_tiled_kernel<false, kPassAll>,
@@ -612,7 +611,7 @@ int launch_interact_tiled(sph_ctx *c, int64_t n, const InteractIn &in, const uin
                                              cudaFuncAttributeMaxDynamicSharedMemorySize, smem));
         SPH_CUDA_TRY(c, cudaFuncSetAttribute(interact_tiled_kernel<true, kPassRemote>,
                                              cudaFuncAttributeMaxDynamicSharedMemorySize, smem));
-        attr_set = true;
+        c->attr_interact = true;
     }
     const int tiles_x = (c->grid.nx + kTBX - 1) / kTBX, tiles_y = (c->grid.ny + kTBY - 1) / kTBY;
     const int64_t tiles = (int64_t)tiles_x * tiles_y * c->grid.nz;

@@ -48,6 +48,15 @@ __global__ void __launch_bounds__(256) radix_hist_kernel(int64_t n, const uint32
     for (int i = threadIdx.x; i < kMaxPasses * kRadix; i += blockDim.x) (&s_hist[0][0])[i] = 0;
     __syncthreads();
     const int lane = threadIdx.x & 31;
+    // keys are only 4-byte aligned by contract (include/sph.h): a scalar head of up to 3 keys
+    // brings the 128-bit loads onto a 16-byte boundary
+    int64_t head = (int64_t)((16 - (reinterpret_cast<uintptr_t>(keys) & 15)) & 15) >> 2;
+    if (head > n) head = n;
+    if (blockIdx.x == 0 && threadIdx.x == 32)
+        for (int64_t i = 0; i < head; ++i)
+            for (int p = 0; p < NP; ++p) atomicAdd(&s_hist[p][(keys[i] >> (p * kRadixBits)) & (kRadix - 1)], 1u);
+    keys += head;
+    n -= head;
     const int64_t n4 = n >> 2;                       // whole 128-bit groups
     const int64_t stride = (int64_t)gridDim.x * blockDim.x;
     // block-uniform trip count (the warp-collective needs full warps), two loads in flight
@@ -293,6 +302,19 @@ __global__ void __launch_bounds__(256) iota_copy_kernel(int64_t n, const uint32_
     if (i < n) { sorted_hash[i] = hash[i]; perm[i] = (uint32_t)i; }
 }
 
+// the opt-in to > 48 KB of dynamic shared memory is per device: once per ctx (a ctx is bound to
+// the device that was current at sph_create)
+static int sort_smem_opt_in(sph_ctx *c)
+{
+    if (c->attr_sort) return SPH_OK;
+    SPH_CUDA_TRY(c, cudaFuncSetAttribute(onesweep_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                         (int)sizeof(SortSmem)));
+    SPH_CUDA_TRY(c, cudaFuncSetAttribute(onesweep_kernel<false>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                         (int)sizeof(SortSmem)));
+    c->attr_sort = true;
+    return SPH_OK;
+}
+
 int launch_sort(sph_ctx *c, int64_t n, const uint32_t *hash, uint32_t *sorted_hash, uint32_t *perm)
 {
     if (n == 0) return SPH_OK;
@@ -319,13 +341,9 @@ int launch_sort(sph_ctx *c, int64_t n, const uint32_t *hash, uint32_t *sorted_ha
     radix_hist_scan_kernel<<<P, kRadix, 0, c->stream>>>(c->hist);
     SPH_CHECK_LAUNCH(c);
 
-    static bool attr_set = false;
-    if (!attr_set) {
-        SPH_CUDA_TRY(c, cudaFuncSetAttribute(onesweep_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                                             (int)sizeof(SortSmem)));
-        SPH_CUDA_TRY(c, cudaFuncSetAttribute(onesweep_kernel<false>, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                                             (int)sizeof(SortSmem)));
-        attr_set = true;
+    {
+        int rc = sort_smem_opt_in(c);
+        if (rc != SPH_OK) return rc;
     }
     // the last pass must land in (sorted_hash, perm): alternate backwards from there
     const uint32_t *kin = hash, *vin = nullptr;
@@ -394,8 +412,10 @@ int launch_partition_by_label(sph_ctx *c, int64_t m, const uint32_t *ids, const 
     SPH_CHECK_LAUNCH(c);
     segment_offsets_kernel<<<1, 64, 0, c->stream>>>(c->hist, n_labels, (uint32_t)m, offsets);
     SPH_CHECK_LAUNCH(c);
-    SPH_CUDA_TRY(c, cudaFuncSetAttribute(onesweep_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                                         (int)sizeof(SortSmem)));
+    {
+        int rc = sort_smem_opt_in(c);
+        if (rc != SPH_OK) return rc;
+    }
     // values = the implicit list indices 0..m-1 (FIRST), so inv_out[k] is entry k's destination
     onesweep_kernel<true><<<(unsigned)tiles, kSortThreads, sizeof(SortSmem), c->stream>>>(
         m, key, nullptr, key_out, val_out, c->hist, c->tile_status, c->tile_counter, 0, dest);

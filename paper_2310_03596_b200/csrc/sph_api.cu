@@ -84,11 +84,15 @@ bool n_ok(const sph_ctx *c, int64_t n) { return c && n >= 0 && n <= c->max_n; }
 
 struct StageTimer {
     sph_ctx *c;
-    int idx = 0;
-    explicit StageTimer(sph_ctx *ctx) : c(ctx) { mark(); }
+    int idx = 0, slot = 0;
+    explicit StageTimer(sph_ctx *ctx) : c(ctx)
+    {
+        if (c->timing.on) slot = (int)(c->timing.count++ % kTimingSlots);
+        mark();
+    }
     void mark()
     {
-        if (c->timing.on) cudaEventRecord(c->timing.ev[idx], c->stream);
+        if (c->timing.on) cudaEventRecord(c->timing.ev[slot][idx], c->stream);
         ++idx;
     }
 };
@@ -127,6 +131,7 @@ int sph_create(sph_ctx **out, const sph_params *p, int64_t max_n, void *cuda_str
     c->last_err = cudaSuccess;
     c->staging_ready = false;
     c->rec_fresh = false;
+    c->attr_sort = c->attr_interact = false;
     memset(&c->staging, 0, sizeof(c->staging));
 
     // grid constants: inv_edge rounded once in fp32 (reading S2)
@@ -156,9 +161,6 @@ int sph_create(sph_ctx **out, const sph_params *p, int64_t max_n, void *cuda_str
     e = cudaMalloc(&c->arena, total);
     if (e != cudaSuccess) { cudaGetLastError(); delete c; return SPH_ENOMEM; }
     carve(c, static_cast<char *>(c->arena), &total);
-    for (int i = 0; i < 9; ++i) {
-        if (cudaEventCreate(&c->timing.ev[i]) != cudaSuccess) { cudaFree(c->arena); delete c; return SPH_ECUDA; }
-    }
     *out = c;
     return SPH_OK;
 }
@@ -167,7 +169,9 @@ int sph_destroy(sph_ctx *c)
 {
     if (!c) return SPH_EINVAL;
     cudaStreamSynchronize(c->stream);
-    for (int i = 0; i < 9; ++i) cudaEventDestroy(c->timing.ev[i]);
+    if (c->timing.created)
+        for (int s = 0; s < kTimingSlots; ++s)
+            for (int i = 0; i < 9; ++i) cudaEventDestroy(c->timing.ev[s][i]);
     if (c->staging_ready) {
         cudaFree(c->staging.posm);
     }
@@ -391,16 +395,34 @@ int sph_step_host(sph_ctx *c, int64_t n, float dt, int32_t steps, const sph_stat
 int sph_enable_timing(sph_ctx *c, int32_t on)
 {
     if (!c) return SPH_EINVAL;
+    if (on && !c->timing.created) {
+        for (int s = 0; s < kTimingSlots; ++s)
+            for (int i = 0; i < 9; ++i) SPH_CUDA_TRY(c, cudaEventCreate(&c->timing.ev[s][i]));
+        c->timing.created = true;
+    }
     c->timing.on = on != 0;
+    c->timing.count = 0;
     return SPH_OK;
 }
 
 int sph_get_timing(sph_ctx *c, float ms[8])
 {
     if (!c || !ms) return SPH_EINVAL;
+    if (!c->timing.created || c->timing.count == 0) return SPH_EINVAL;
     SPH_CUDA_TRY(c, cudaStreamSynchronize(c->stream));
-    for (int i = 0; i < 7; ++i) SPH_CUDA_TRY(c, cudaEventElapsedTime(&ms[i], c->timing.ev[i], c->timing.ev[i + 1]));
-    SPH_CUDA_TRY(c, cudaEventElapsedTime(&ms[7], c->timing.ev[0], c->timing.ev[7]));
+    const int m = (int)(c->timing.count < kTimingSlots ? c->timing.count : kTimingSlots);
+    for (int i = 0; i < 8; ++i) ms[i] = 0.f;
+    for (int k = 0; k < m; ++k) {   // the m most recent steps
+        const int s = (int)((c->timing.count - 1 - k) % kTimingSlots);
+        float t;
+        for (int i = 0; i < 7; ++i) {
+            SPH_CUDA_TRY(c, cudaEventElapsedTime(&t, c->timing.ev[s][i], c->timing.ev[s][i + 1]));
+            ms[i] += t / (float)m;
+        }
+        SPH_CUDA_TRY(c, cudaEventElapsedTime(&t, c->timing.ev[s][0], c->timing.ev[s][7]));
+        ms[7] += t / (float)m;
+    }
+    c->timing.count = 0;
     return SPH_OK;
 }
 

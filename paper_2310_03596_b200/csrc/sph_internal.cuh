@@ -42,9 +42,14 @@ struct Consts {
     float K, G;
 };
 
+// Stage events of the most recent steps: a ring of kTimingSlots event sets so that a caller can
+// time many steps back to back without a host sync in between (sph_get_timing averages them).
+constexpr int kTimingSlots = 32;
 struct Timing {
     bool on = false;
-    cudaEvent_t ev[9] = {};
+    bool created = false;
+    int64_t count = 0;                       // steps recorded since the last sph_get_timing
+    cudaEvent_t ev[kTimingSlots][9] = {};
 };
 
 }  // namespace sphb
@@ -83,6 +88,7 @@ struct sph_ctx {
     float4 *rec_D;
     void *bal;                                // control block of the balancing sweep (balance.cu)
     bool rec_fresh;                           // rec_B/C/D already hold the records of `sorted` (written by reorder)
+    bool attr_sort, attr_interact;            // >48 KB dynamic shared memory opted in on THIS ctx's device
     // host-API staging (lazy)
     sph_state staging;
     bool staging_ready;

@@ -25,6 +25,7 @@ SPH_OK, SPH_EINVAL, SPH_ECUDA, SPH_ENOMEM = 0, -1, -2, -3
 GARBAGE_HASH = 0xFFFFFFFF
 MAX_OWNERS = 32
 FLAG_INTERACT_DIRECT = 1
+TIMING_SLOTS = 32          # steps held by the library's ring of stage events (sph_get_timing)
 
 EXPORTS = (
     "sph_create", "sph_destroy", "sph_hash", "sph_sort", "sph_reorder", "sph_cell_ranges",

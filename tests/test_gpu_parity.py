@@ -178,6 +178,24 @@ def test_sort_random_keys_many_tiles(sph, oracle):
     ctx.close()
 
 
+def test_sort_from_unaligned_key_pointer(sph, oracle):
+    # include/sph.h promises 4-byte alignment for hash arrays: sort from views offset by 1, 2, 3 keys
+    rng = np.random.default_rng(6)
+    dims = np.array([79, 79, 79], np.int32)
+    cells = int(np.prod(dims.astype(np.int64)))
+    n = 3 * 8192 + 77
+    ctx = sph.Context(np.zeros(3, np.float32), dims, 1.3, max_n=n)
+    buf = torch.from_numpy(rng.integers(0, cells, n + 3).astype(np.uint32).view(np.int32)).cuda()
+    for off in (1, 2, 3):
+        view = buf[off:off + n]
+        assert view.data_ptr() % 16 == 4 * off
+        sh, perm = ctx.sph_sort(view)
+        rs, rp = oracle.sort(parity.u32(view))
+        np.testing.assert_array_equal(parity.u32(sh), rs)
+        np.testing.assert_array_equal(parity.u32(perm), rp)
+    ctx.close()
+
+
 def test_step_host_end_to_end(sph, oracle):
     w = wl.t1b(side=12)
     ctx = sph.Context.for_workload(w)
