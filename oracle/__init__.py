@@ -53,6 +53,9 @@ def _load():
     lib.orc_interact_split.argtypes = [i64, vp, vp, vp, vp, vp, vp, vp, f32, f32, f32, vp, C.c_int,
                                        i64, vp, vp, vp, vp, vp, vp]
     lib.orc_interact_split.restype = None
+    lib.orc_interact_varh.argtypes = [i64, vp, vp, vp, vp, vp, vp, vp, vp, f32, f32, f32, vp, C.c_int,
+                                      i64, vp, vp, vp, vp, vp, vp]
+    lib.orc_interact_varh.restype = None
     lib.orc_integrate.argtypes = [i64, f64, vp, vp, vp, vp, vp, vp, vp, vp, vp]
     lib.orc_integrate.restype = None
     _lib = lib
@@ -256,6 +259,41 @@ def interact_split(posm, velr, sig, sorted_hash, dims, cell_start, cell_end, h, 
     return Rates(drho, L, acc, dsig, int(pc.value))
 
 
+def interact_varh(posm, velr, sig, hp, sorted_hash, dims, cell_start, cell_end, hmax, K, G, owner=None, which=0,
+                  idx=None) -> Rates:
+    """O7 with a smoothing length per particle (sph_oracle.c orc_interact_varh; PAPER.md:13, 54;
+    readings H1-H3): pair length h_ij = (h_i + h_j) / 2, bucket grid on hmax.  All arrays in sorted
+    order; owner / which select a split pass, idx a sample of sorted positions."""
+    posm = _c(posm, np.float32)
+    velr = _c(velr, np.float32)
+    sig = _c(sig, np.float32)
+    hp = _c(hp, np.float32)
+    n = posm.shape[0]
+    assert hp.shape == (n,)
+    if owner is not None:
+        owner = _c(owner, np.int32)
+    sorted_hash = _c(sorted_hash, np.uint32)
+    dims = _c(dims, np.int32)
+    cell_start = _c(cell_start, np.uint32)
+    cell_end = _c(cell_end, np.uint32)
+    if idx is not None:
+        idx = _c(idx, np.int64)
+        m = idx.shape[0]
+    else:
+        m = n
+    drho = np.zeros(m, np.float64)
+    L = np.zeros((m, 3, 3), np.float64)
+    acc = np.zeros((m, 3), np.float64)
+    dsig = np.zeros((m, 6), np.float64)
+    pc = C.c_int64(0)
+    _load().orc_interact_varh(n, _p(posm), _p(velr), _p(sig), _p(hp), _p(sorted_hash), _p(dims),
+                              _p(cell_start), _p(cell_end), np.float32(hmax), np.float32(K), np.float32(G),
+                              _p(owner) if owner is not None else None, int(which),
+                              m if idx is not None else 0, _p(idx) if idx is not None else None,
+                              _p(drho), _p(L), _p(acc), _p(dsig), C.byref(pc))
+    return Rates(drho, L, acc, dsig, int(pc.value))
+
+
 def integrate(dt, posm, velr, sig, drho, acc, dsig):
     posm = _c(posm, np.float32)
     velr = _c(velr, np.float32)
@@ -288,10 +326,11 @@ class StepResult:
     sig: np.ndarray | None
 
 
-def step(posm, velr, sig, owner, origin, dims, h, K, G, n_owners, dt, floats=True) -> StepResult:
+def step(posm, velr, sig, owner, origin, dims, h, K, G, n_owners, dt, floats=True, hp=None) -> StepResult:
     """One iteration from an id-ordered fp32 state.  sig is [6, n].
 
     floats=False stops after the integer stages (steps a and c and the boundary set).
+    hp = per-particle smoothing lengths in id order (None = uniform h); h is then h_max (H1).
     """
     posm = _c(posm, np.float32)
     velr = _c(velr, np.float32)
@@ -308,7 +347,10 @@ def step(posm, velr, sig, owner, origin, dims, h, K, G, n_owners, dt, floats=Tru
     if not floats:
         return StepResult(hsh, sh, perm, cs, ce, ch, bids, ocnt, None, None, None, None)
     sp, sv, ss = posm[perm], velr[perm], np.ascontiguousarray(sig[:, perm])
-    rates = interact(sp, sv, ss, sh, dims, cs, ce, h, K, G)         # steps e, f
+    if hp is None:
+        rates = interact(sp, sv, ss, sh, dims, cs, ce, h, K, G)     # steps e, f
+    else:
+        rates = interact_varh(sp, sv, ss, _c(hp, np.float32)[perm], sh, dims, cs, ce, h, K, G)
     po_s, vo_s, so_s = integrate(dt, sp, sv, ss, rates.drho, rates.acc, rates.dsig)  # step g
     n = posm.shape[0]
     po = np.empty((n, 4)); vo = np.empty((n, 4)); so = np.empty((6, n))

@@ -266,6 +266,7 @@ static void orc_interact_impl(int64_t n, const float *posm, const float *velr, c
                   const uint32_t *sorted_hash, const int32_t *dims, const uint32_t *cell_start,
                   const uint32_t *cell_end, float h_f32, float K_f32, float G_f32,
                   int64_t n_idx, const int64_t *idx, const int32_t *owner, int which,
+                  const float *hp,
                   double *drho, double *L, double *acc, double *dsig, int64_t *pair_count)
 {
     const double h = (double)h_f32, K = (double)K_f32, G = (double)G_f32;
@@ -299,9 +300,13 @@ static void orc_interact_impl(int64_t n, const float *posm, const float *velr, c
                         const double xij[3] = { xi[0] - posm[4 * j + 0], xi[1] - posm[4 * j + 1],
                                                 xi[2] - posm[4 * j + 2] };
                         const double r2 = xij[0] * xij[0] + xij[1] * xij[1] + xij[2] * xij[2];
-                        if (!(r2 < support2)) continue;
+                        /* O7h (reading H2): per-particle smoothing lengths enter through the
+                         * symmetrised pair length h_ij = (h_i + h_j) / 2, support 2 h_ij */
+                        const double hij = hp ? 0.5 * ((double)hp[i] + (double)hp[j]) : h;
+                        const double sup2 = hp ? (2.0 * hij) * (2.0 * hij) : support2;
+                        if (!(r2 < sup2)) continue;
                         ++pairs;
-                        const double F = orc_kernel_F(sqrt(r2), h);
+                        const double F = orc_kernel_F(sqrt(r2), hij);
                         const double mj = posm[4 * j + 3], rhoj = velr[4 * j + 3];
                         const double gW[3] = { F * xij[0], F * xij[1], F * xij[2] };
                         const double vij[3] = { vi[0] - velr[4 * j + 0], vi[1] - velr[4 * j + 1],
@@ -328,8 +333,10 @@ static void orc_interact_impl(int64_t n, const float *posm, const float *velr, c
                         const double xij[3] = { xi[0] - posm[4 * j + 0], xi[1] - posm[4 * j + 1],
                                                 xi[2] - posm[4 * j + 2] };
                         const double r2 = xij[0] * xij[0] + xij[1] * xij[1] + xij[2] * xij[2];
-                        if (!(r2 < support2)) continue;
-                        const double F = orc_kernel_F(sqrt(r2), h);
+                        const double hij = hp ? 0.5 * ((double)hp[i] + (double)hp[j]) : h;
+                        const double sup2 = hp ? (2.0 * hij) * (2.0 * hij) : support2;
+                        if (!(r2 < sup2)) continue;
+                        const double F = orc_kernel_F(sqrt(r2), hij);
                         const double mj = posm[4 * j + 3], rhoj = velr[4 * j + 3];
                         double sj[3][3];
                         orc_sym_load(sig, n, j, sj);
@@ -378,7 +385,7 @@ void orc_interact(int64_t n, const float *posm, const float *velr, const float *
                   double *drho, double *L, double *acc, double *dsig, int64_t *pair_count)
 {
     orc_interact_impl(n, posm, velr, sig, sorted_hash, dims, cell_start, cell_end, h_f32, K_f32, G_f32,
-                      n_idx, idx, NULL, 0, drho, L, acc, dsig, pair_count);
+                      n_idx, idx, NULL, 0, NULL, drho, L, acc, dsig, pair_count);
 }
 
 /* NEXT-3: steps e (which = 1) and f (which = 2) as separate passes; owner is in sorted order.
@@ -390,7 +397,26 @@ void orc_interact_split(int64_t n, const float *posm, const float *velr, const f
                         double *drho, double *L, double *acc, double *dsig, int64_t *pair_count)
 {
     orc_interact_impl(n, posm, velr, sig, sorted_hash, dims, cell_start, cell_end, h_f32, K_f32, G_f32,
-                      n_idx, idx, owner, which, drho, L, acc, dsig, pair_count);
+                      n_idx, idx, owner, which, NULL, drho, L, acc, dsig, pair_count);
+}
+
+/* NEXT-4, second half ("cubic buckets of size 2h with h the maximum
+ * smoothing length of the particles"; "multiple particle types with different
+ * smoothing lengths"): O7 with a smoothing length per particle.  Readings:
+ *   H1  the bucket grid is built on h_max (the h of orc_hash / cell tables), every hp[i] <= h_max;
+ *   H2  a pair uses the symmetrised length h_ij = (h_i + h_j) / 2 in fp64: W(r, h_ij), neighbours
+ *       are the stencil particles with r < 2 h_ij (inside the 27 buckets because h_ij <= h_max);
+ *       the pair force stays antisymmetric, so momentum is still conserved exactly;
+ *   H3  everything else (sums, O8) as in orc_interact; uniform hp == h reproduces it bit for bit.
+ * hp [n] in sorted order; owner / which as in orc_interact_split (owner may be NULL with which = 0). */
+void orc_interact_varh(int64_t n, const float *posm, const float *velr, const float *sig,
+                       const float *hp, const uint32_t *sorted_hash, const int32_t *dims,
+                       const uint32_t *cell_start, const uint32_t *cell_end, float hmax_f32, float K_f32,
+                       float G_f32, const int32_t *owner, int which, int64_t n_idx, const int64_t *idx,
+                       double *drho, double *L, double *acc, double *dsig, int64_t *pair_count)
+{
+    orc_interact_impl(n, posm, velr, sig, sorted_hash, dims, cell_start, cell_end, hmax_f32, K_f32, G_f32,
+                      n_idx, idx, owner, which, hp, drho, L, acc, dsig, pair_count);
 }
 
 /* ------------------------------------------------------------------------------------------

@@ -187,6 +187,31 @@ def t1b(side=16, seed=1100):
     return w
 
 
+def particle_h(w: Workload, kind=("species", 2, 0.75), seed=2000) -> np.ndarray:
+    """Per-particle smoothing lengths in id order for the non-uniform-h cases (SURVEY.md 8(f)
+    NEXT-4; "h the maximum smoothing length of the particles", PAPER.md:54 particle
+    types "with different smoothing lengths").  The grid of `w` stays built on w.h = h_max.
+    kind: ("species", k, fmin)  particle type = seeded uniform in 0..k-1, h = h_max (1 - (1 - fmin) type / (k - 1))
+          ("checker", f)        h_max on even lattice sites (id parity along x, y, z), f h_max on odd ones
+          ("uniform",)          every particle h_max
+          ("random", fmin)      h_max U(fmin, 1)"""
+    n, hmax = w.n, np.float32(w.h)
+    rng = np.random.Generator(np.random.PCG64(seed))
+    if kind[0] == "uniform":
+        return np.full(n, hmax, np.float32)
+    if kind[0] == "species":
+        k, fmin = int(kind[1]), float(kind[2])
+        typ = rng.integers(0, k, n)
+        return (hmax * (1.0 - (1.0 - fmin) * typ / max(k - 1, 1))).astype(np.float32)
+    if kind[0] == "checker":
+        site = np.rint(w.posm[:, :3]).astype(np.int64)
+        odd = (site.sum(1) & 1).astype(bool)
+        return np.where(odd, np.float32(kind[1]) * hmax, hmax).astype(np.float32)
+    if kind[0] == "random":
+        return (hmax * rng.uniform(float(kind[1]), 1.0, n)).astype(np.float32)
+    raise ValueError(kind)
+
+
 def _config3(seed, scale=1.0):
     """Plate [0,400)x[0,400)x[0,100) U 8 cylinders (axis z, radius 40, z in [100,250)), centres
     uniform in [40,360]^2 rejecting overlaps.  `scale` shrinks every length (tests)."""

@@ -551,6 +551,92 @@ def test_split_passes_sum_to_the_single_pass_and_match_bruteforce():
     np.testing.assert_array_equal(fs.dsig, f.dsig[pick])
 
 
+# ----------------------------------------------------------------------------- NEXT-4: per-particle h
+def _sorted_with_h(w, hp):
+    r, sp, sv, ss, so = sorted_view(w)
+    return r, sp, sv, ss, so, hp[r.perm]
+
+
+def test_varh_uniform_reduces_to_the_plain_loops_bit_for_bit():
+    """H3: with every h_i = h the pair length (h + h) / 2 is h exactly: same bits as orc_interact."""
+    w = W.t1b(10, 1106)
+    r, sp, sv, ss, so, sh = _sorted_with_h(w, W.particle_h(w, ("uniform",)))
+    a = orc.interact(sp, sv, ss, r.sorted_hash, w.dims, r.cell_start, r.cell_end, w.h, w.K, w.G)
+    b = orc.interact_varh(sp, sv, ss, sh, r.sorted_hash, w.dims, r.cell_start, r.cell_end, w.h, w.K, w.G)
+    assert a.pair_count == b.pair_count
+    for name in ("drho", "L", "acc", "dsig"):
+        assert np.array_equal(getattr(a, name), getattr(b, name)), name
+
+
+@pytest.mark.parametrize("kind", [("species", 2, 0.75), ("species", 3, 0.6), ("random", 0.5)])
+def test_varh_against_dense_evaluation_by_distance(kind):
+    """H2: pair length h_ij = (h_i + h_j) / 2, neighbours r < 2 h_ij found by distance alone in an
+    O(N^2) numpy evaluation (no buckets): every output of both loops, the pair count, and exact
+    momentum conservation (the pair force stays antisymmetric)."""
+    w = W.t1b(10, 1107)
+    w.posm[:, 3] = (1.0 + 0.2 * np.random.default_rng(2).random(w.n)).astype(np.float32)
+    hp = W.particle_h(w, kind)
+    assert hp.max() <= w.h and hp.min() < w.h
+    r, sp, sv, ss, so, sh = _sorted_with_h(w, hp)
+    got = orc.interact_varh(sp, sv, ss, sh, r.sorted_hash, w.dims, r.cell_start, r.cell_end, w.h, w.K, w.G)
+    x = sp[:, :3].astype(np.float64); m = sp[:, 3].astype(np.float64)
+    v = sv[:, :3].astype(np.float64); rho = sv[:, 3].astype(np.float64)
+    sg = ss.astype(np.float64)
+    S = np.empty((w.n, 3, 3))
+    S[:, 0, 0], S[:, 1, 1], S[:, 2, 2] = sg[0], sg[1], sg[2]
+    S[:, 0, 1] = S[:, 1, 0] = sg[3]; S[:, 0, 2] = S[:, 2, 0] = sg[4]; S[:, 1, 2] = S[:, 2, 1] = sg[5]
+    Sr = S / (rho ** 2)[:, None, None]
+    hij = 0.5 * (sh.astype(np.float64)[:, None] + sh.astype(np.float64)[None, :])
+    xij = x[:, None, :] - x[None, :, :]
+    rr = np.sqrt((xij ** 2).sum(-1))
+    nb = (rr < 2 * hij) & ~np.eye(w.n, dtype=bool)
+    alpha = 21.0 / (16.0 * np.pi * hij ** 3)
+    Fm = np.where(nb, -(5.0 * alpha / hij ** 2) * (1 - rr / (2 * hij)) ** 3, 0.0)
+    gW = Fm[..., None] * xij
+    vij = v[:, None, :] - v[None, :, :]
+    drho = (m[None, :] * (vij * gW).sum(-1)).sum(1)
+    Ld = np.einsum("j,ija,ijb->iab", m / rho, -vij, gW)
+    accd = np.einsum("j,ijab,ijb->ia", m, Sr[:, None] + Sr[None, :], gW)
+    for name, ref in (("drho", drho), ("L", Ld), ("acc", accd)):
+        assert np.max(np.abs(getattr(got, name) - ref)) <= 1e-11 * np.max(np.abs(ref)), name
+    assert got.pair_count == int(nb.sum())
+    f = m[:, None] * got.acc
+    assert np.abs(f.sum(0)).max() <= 1e-12 * np.abs(f).sum() and np.abs(f).sum() > 0
+    # fewer neighbours than with the maximum length everywhere
+    full = orc.interact(sp, sv, ss, r.sorted_hash, w.dims, r.cell_start, r.cell_end, w.h, w.K, w.G)
+    assert got.pair_count < full.pair_count
+
+
+def test_varh_two_species_lattice_neighbour_counts():
+    """Un-jittered unit lattice, h = 1.3 on even sites and 1.0 on odd ones (checkerboard): the
+    neighbours of an interior particle follow from integer arithmetic alone.  Even-even pairs see
+    r^2 < 6.76 (h_ij = 1.3), odd-odd pairs r^2 < 4 (h_ij = 1.0), mixed pairs r^2 < 5.29
+    (h_ij = 1.15); a lattice vector connects equal parities iff its coordinate sum is even."""
+    side = 12
+    w = W.lattice_block(side, side, side, 0.0, 5, owners=("single",))
+    hp = W.particle_h(w, ("checker", 1.0 / 1.3))
+    r, sp, sv, ss, so, sh = _sorted_with_h(w, hp)
+    got = orc.interact_varh(sp, sv, ss, sh, r.sorted_hash, w.dims, r.cell_start, r.cell_end, w.h, w.K, w.G,
+                            idx=np.arange(w.n))
+    d = np.arange(-3, 4)
+    DX, DY, DZ = np.meshgrid(d, d, d, indexing="ij")
+    r2 = (DX ** 2 + DY ** 2 + DZ ** 2).ravel()
+    same = ((DX + DY + DZ) % 2 == 0).ravel()
+    nz = r2 > 0
+    n_even = int((nz & same & (r2 < 6.76)).sum() + (nz & ~same & (r2 < 5.29)).sum())
+    n_odd = int((nz & same & (r2 < 4.0)).sum() + (nz & ~same & (r2 < 5.29)).sum())
+    # per-particle neighbour counts through the single-particle form of the oracle
+    site = np.rint(sp[:, :3]).astype(int)
+    interior = np.all((site >= 3) & (site < side - 3), axis=1)
+    for parity, expect in ((0, n_even), (1, n_odd)):
+        pick = np.nonzero(interior & ((site.sum(1) & 1) == parity))[0][:5]
+        for i in pick:
+            one = orc.interact_varh(sp, sv, ss, sh, r.sorted_hash, w.dims, r.cell_start, r.cell_end, w.h, w.K,
+                                    w.G, idx=np.array([i]))
+            assert one.pair_count == expect, (parity, one.pair_count, expect)
+    assert n_even != n_odd
+
+
 # ----------------------------------------------------------------------------- NEXT-2: balancing
 def test_balance_hand_worked_example_golden():
     """PAPER.md:36 on four particles, worked by hand (tests/golden/balancing_worked_example.txt)."""
