@@ -52,7 +52,7 @@ typedef struct sph_ctx sph_ctx;      /* opaque */
 typedef struct {
     float    origin[3];  /* lower corner of the bucket grid (reading S3)                        */
     int32_t  dims[3];    /* nx, ny, nz buckets; nx*ny*nz < 2^32 - 1                              */
-    float    h;          /* uniform smoothing length; bucket edge = support = 2h   */
+    float    h;          /* smoothing length (the MAXIMUM one with sph_*_varh); bucket edge = 2h   */
     float    K, G;       /* bulk / shear modulus of the linear-elastic law (BASELINE.json cfgs)  */
     int32_t  n_owners;   /* 1 .. SPH_MAX_OWNERS                                                  */
     uint32_t flags;      /* SPH_FLAG_* or 0                                                      */
@@ -208,6 +208,28 @@ int sph_balance(sph_ctx *ctx, int64_t n, const float *posm, int32_t *owner, int3
 int sph_balance_types(sph_ctx *ctx, int64_t n, const float *posm, int32_t *owner, const int32_t *ptype,
                       int32_t n_types, double alpha, int32_t hmax, int32_t *bal_hash,
                       unsigned long long *swapped);
+
+/* NEXT-4, second half -- per-particle smoothing lengths ("cubic
+ * buckets of size 2h with h the maximum smoothing length of the particles"; PAPER.md:54 particle
+ * types "with different smoothing lengths").  Readings H1-H3: the bucket grid
+ * stays the one of sph_params.h, which is now h_max (every h[i] must be in (0, h_max]; larger
+ * values lose neighbours outside the 27 buckets, not checked); a pair uses the symmetrised length
+ * h_ij = (h_i + h_j) / 2: W(r, h_ij), neighbours = stencil particles with r < 2 h_ij; all sums and
+ * the stress rate as in sph_interact.  Every h[i] == sph_params.h gives sph_interact's result up
+ * to rounding.  Stages 1-3 do not depend on h.
+ * sph_interact_varh: sorted_h dev [n] in sorted order; which = 0 all neighbours, 1 / 2 = the split
+ * passes of sph_interact_split; the rest as sph_interact (pair_count is zeroed by the call).
+ * sph_step_varh: h dev [n] in ID order (read only; smoothing lengths do not evolve); the rest as
+ * sph_step. */
+int sph_interact_varh(sph_ctx *ctx, int64_t n, const sph_state *sorted, const float *sorted_h,
+                      const uint32_t *sorted_hash, const uint32_t *cell_start, const uint32_t *cell_end,
+                      int32_t which, float *drho, float *acc, float *const dsig[6],
+                      unsigned long long *pair_count);
+int sph_step_varh(sph_ctx *ctx, int64_t n, float dt, const sph_state *state, const float *h, uint32_t *hash,
+                  uint32_t *sorted_hash, uint32_t *perm, uint32_t *cell_start, uint32_t *cell_end,
+                  uint32_t *comm_hash, uint32_t *boundary_ids, uint32_t *boundary_count,
+                  uint32_t *owner_counts, float *drho, float *acc, float *const dsig[6],
+                  unsigned long long *pair_count);
 
 /* End-to-end variant with HOST buffers (pinned memory recommended): uploads the id-ordered state,
  * runs `steps` iterations, downloads the state, the boundary list of the last step and the

@@ -8,7 +8,7 @@ namespace sphb {
 int launch_interact(sph_ctx *c, int64_t n, const sph_state *sorted, const uint32_t *sorted_hash,
                     const uint32_t *cs, const uint32_t *ce, float *drho, float *acc,
                     float *const dsig[6], unsigned long long *pair_count, const sph_state *fuse_out,
-                    const uint32_t *perm, float dt, int mode)
+                    const uint32_t *perm, float dt, int mode, const float *sorted_h)
 {
     if (n == 0) return SPH_OK;
     InteractIn in;
@@ -16,6 +16,7 @@ int launch_interact(sph_ctx *c, int64_t n, const sph_state *sorted, const uint32
     in.posm = reinterpret_cast<const float4 *>(sorted->posm);
     in.velr = reinterpret_cast<const float4 *>(sorted->velr);
     in.owner = sorted->owner;
+    in.h = sorted_h;
     out.drho = drho;   // NULL (with fuse_out set): the rates are not stored
     out.acc = reinterpret_cast<float4 *>(acc);
     for (int i = 0; i < 6; ++i) { in.sig[i] = sorted->sig[i]; out.dsig[i] = dsig ? dsig[i] : nullptr; }

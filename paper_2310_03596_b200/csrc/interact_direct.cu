@@ -34,8 +34,10 @@ int launch_interact_direct(sph_ctx *c, int64_t n, const InteractIn &in, const ui
                            const uint32_t *cs, const uint32_t *ce, const InteractOut &out,
                            unsigned long long *pair_count, int mode)
 {
+    Consts kc = c->consts;
+    if (in.h) kc.cF = kc.cF_varh;   // per-particle smoothing lengths: h_ij^-5 is applied per pair
     interact_direct_kernel<<<div_up(n, 128), 128, 0, c->stream>>>(n, in, sorted_hash, cs, ce, c->grid,
-                                                                  c->consts, out, pair_count, mode);
+                                                                  kc, out, pair_count, mode);
     SPH_CHECK_LAUNCH(c);
     return SPH_OK;
 }

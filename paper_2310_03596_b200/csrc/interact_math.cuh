@@ -15,6 +15,7 @@ struct InteractIn {
     const float4 *posm, *velr;
     const float *sig[6];
     const int32_t *owner;   // sorted owner labels; only read by the split passes (NEXT-3)
+    const float *h;         // sorted per-particle smoothing lengths (NEXT-4), NULL = uniform
 };
 
 // Which neighbours a pass takes: 0 = all (steps e and f as one loop),
@@ -41,6 +42,20 @@ __device__ __forceinline__ float sqrt_approx(float x)
     return y;
 }
 
+// NEXT-4 (per-particle smoothing lengths, reading H2): pair length h_ij = (h_i + h_j) / 2.
+// Returns 1 / (h_i + h_j) = 1 / (2 h_ij) (MUFU.RCP + one Newton step) and h_ij^-5 in *ih5:
+// grad W = -(105 / 16 pi) h_ij^-5 (1 - r / 2 h_ij)^3 x_ij, the constant is applied per particle.
+__device__ __forceinline__ float pair_inv_2h(float hi, float hj, float *ih5)
+{
+    const float hs = hi + hj;
+    float inv;
+    asm("rcp.approx.ftz.f32 %0, %1;" : "=f"(inv) : "f"(hs));
+    inv = inv * fmaf(-hs, inv, 2.0f);
+    const float ih = 2.0f * inv, ih2 = ih * ih;
+    *ih5 = ih2 * ih2 * ih;
+    return inv;
+}
+
 struct PairAccum {
     float dr;          // sum dv . mx
     float L[9];        // sum dv_a * wx_b
@@ -55,13 +70,14 @@ struct PairAccum {
         for (int i = 0; i < 3; ++i) { g[i] = 0.f; a[i] = 0.f; }
     }
     // S = (xx, yy, zz, xy, xz, yz) of sigma_j / rho_j^2
+    // scale = 1 (uniform h: the constant cF is applied once per particle) or h_ij^-5 (NEXT-4)
     __device__ __forceinline__ void add(float dx, float dy, float dz, float r2, float mj, float Vj,
                                         float dvx, float dvy, float dvz, const float (&S)[6],
-                                        float half_inv_h)
+                                        float half_inv_h, float scale = 1.0f)
     {
         const float r = sqrt_approx(r2);              // coincident particles: r = 0, gradW = 0 (S15)
         const float t = fmaxf(fmaf(r, -half_inv_h, 1.0f), 0.0f);  // W = 0 beyond the support
-        const float F = t * t * t;
+        const float F = t * t * t * scale;
         const float wm = mj * F, wV = Vj * F;
         const float mx = wm * dx, my = wm * dy, mz = wm * dz;
         const float wx = wV * dx, wy = wV * dy, wz = wV * dz;
@@ -143,18 +159,29 @@ struct PairAccum2 {
         dr2 = Lx = Ly = Lz = Lc = g2 = a2 = az2 = 0ull;
         drz = Lzz = gz = azz = 0.f;
     }
-    // tp = target position (tile-local), tv = target velocity; pa..pd = the neighbour record
+    // tp = target position (tile-local), tv = target velocity; pa..pd = the neighbour record.
+    // VH (NEXT-4): C.z carries h_j instead of the second copy of Sxy, hi = the target's length;
+    // returns r^2 - (h_i + h_j)^2 + support2-free form: see the caller (pair counting).
+    template <bool VH = false>
     __device__ __forceinline__ float add(f32x2 tpxy, float tpz, f32x2 tvxy, float tvz, const float4 &pa,
                                          const float4 &pb, const float4 &pc, const float4 &pd,
-                                         float neg_half_inv_h)
+                                         float neg_half_inv_h, float hi = 0.f)
     {
         const f32x2 dxy = sub2(tpxy, pk(pa.x, pa.y));
         const float dz = tpz - pa.z;
         const f32x2 sq = mul2(dxy, dxy);
         const float r2 = fmaf(dz, dz, lo_of(sq)) + hi_of(sq);
         const float r = sqrt_approx(r2);              // coincident particles: r = 0, gradW = 0 (S15)
-        const float t = fmaxf(fmaf(r, neg_half_inv_h, 1.0f), 0.0f);  // W = 0 beyond the support
-        const float F = t * t * t;
+        float F;
+        if (VH) {
+            float ih5;
+            const float inv = pair_inv_2h(hi, pc.z, &ih5);
+            const float t = fmaxf(fmaf(r, -inv, 1.0f), 0.0f);     // W = 0 beyond 2 h_ij
+            F = t * t * t * ih5;
+        } else {
+            const float t = fmaxf(fmaf(r, neg_half_inv_h, 1.0f), 0.0f);  // W = 0 beyond the support
+            F = t * t * t;
+        }
         const f32x2 wmV = mul2(bc(F), pk(pd.z, pd.w));            // (m F, V F)
         const f32x2 mxy = mul2(bc(lo_of(wmV)), dxy);              // m F (dx, dy)
         const f32x2 wxy = mul2(bc(hi_of(wmV)), dxy);              // V F (dx, dy)
@@ -172,7 +199,7 @@ struct PairAccum2 {
         g2 = add2(g2, mxy);
         gz += mz;
         a2 = fma2(bc(lo_of(mxy)), pk(pc.x, pc.y), a2);
-        a2 = fma2(bc(hi_of(mxy)), pk(pc.z, pc.w), a2);
+        a2 = fma2(bc(hi_of(mxy)), pk(VH ? pc.y : pc.z, pc.w), a2);
         a2 = fma2(bc(mz), pk(pd.x, pd.y), a2);
         az2 = fma2(pk(pd.x, pd.y), mxy, az2);
         azz = fmaf(pb.w, mz, azz);
@@ -271,6 +298,7 @@ __device__ __forceinline__ uint32_t direct_particle(int64_t i, int cx, int cy, i
                                                     int mode = kPassAll)
 {
     const int32_t oi = mode != kPassAll ? in.owner[i] : 0;
+    const float hi = in.h ? in.h[i] : 0.f;   // NEXT-4: per-particle smoothing length
     const float4 pi = in.posm[i];
     const float4 vi = in.velr[i];
     PairAccum A;
@@ -290,7 +318,13 @@ __device__ __forceinline__ uint32_t direct_particle(int64_t i, int cx, int cy, i
                 const float dx = pi.x - pj.x, dy_ = pi.y - pj.y, dz_ = pi.z - pj.z;
                 const float r2 = dx * dx + dy_ * dy_ + dz_ * dz_;
                 if (mode != kPassAll && ((in.owner[j] == oi) != (mode == kPassLocal))) continue;
-                if (r2 < k.support2 && j != (uint32_t)i) {
+                float sup2 = k.support2, hinv = k.half_inv_h, scale = 1.0f;
+                if (in.h) {   // pair length h_ij = (h_i + h_j) / 2, support 2 h_ij (reading H2)
+                    const float hs = hi + in.h[j];
+                    sup2 = hs * hs;
+                    hinv = pair_inv_2h(hi, in.h[j], &scale);
+                }
+                if (r2 < sup2 && j != (uint32_t)i) {
                     const float4 vj = in.velr[j];
                     const float inv_rho = 1.0f / vj.w;
                     const float Vj = pj.w * inv_rho;
@@ -299,7 +333,7 @@ __device__ __forceinline__ uint32_t direct_particle(int64_t i, int cx, int cy, i
 #pragma unroll
                     for (int c = 0; c < 6; ++c) Sj[c] = in.sig[c][j] * ir2;
                     A.add(dx, dy_, dz_, r2, pj.w, Vj, vj.x - vi.x, vj.y - vi.y, vj.z - vi.z, Sj,
-                          k.half_inv_h);
+                          hinv, scale);
                     ++pairs;
                 }
             }

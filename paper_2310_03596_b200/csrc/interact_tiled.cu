@@ -65,6 +65,7 @@ __global__ void __launch_bounds__(256)
 pack_kernel(int64_t n, InteractIn in, float4 *__restrict__ B, float4 *__restrict__ C,
             float4 *__restrict__ D)
 {
+    // (NEXT-4: with per-particle smoothing lengths C.z carries h instead of the second Sxy)
     const int64_t k = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
     if (k >= n) return;
     const float m = in.posm[k].w;
@@ -73,7 +74,7 @@ pack_kernel(int64_t n, InteractIn in, float4 *__restrict__ B, float4 *__restrict
     const float ir2 = inv_rho * inv_rho;
     const float sxy = in.sig[3][k] * ir2;
     B[k] = make_float4(v.x, v.y, v.z, in.sig[2][k] * ir2);
-    C[k] = make_float4(in.sig[0][k] * ir2, sxy, sxy, in.sig[1][k] * ir2);
+    C[k] = make_float4(in.sig[0][k] * ir2, sxy, in.h ? in.h[k] : sxy, in.sig[1][k] * ir2);
     D[k] = make_float4(in.sig[4][k] * ir2, in.sig[5][k] * ir2, m, m * inv_rho);
 }
 
@@ -178,7 +179,7 @@ __device__ __forceinline__ float4 ld_rec(const float4 *base, uint32_t e16)
     return *reinterpret_cast<const float4 *>(reinterpret_cast<const char *>(base) + e16);
 }
 
-template <bool kCount, int kMode>
+template <bool kCount, int kMode, bool kVarH>
 __global__ void __launch_bounds__(kTW * 32, 2)
 interact_tiled_kernel(Packed rec, InteractIn in, const uint32_t *__restrict__ cs,
                       const uint32_t *__restrict__ ce, Grid g, Consts k, InteractOut out,
@@ -328,7 +329,7 @@ interact_tiled_kernel(Packed rec, InteractIn in, const uint32_t *__restrict__ cs
             if (tid < 8) {
                 sm.A[kDummy + tid] = make_float4(1e18f, 1e18f, 1e18f, 3e36f);
                 sm.B[kDummy + tid] = make_float4(0.f, 0.f, 0.f, 0.f);
-                sm.C[kDummy + tid] = make_float4(0.f, 0.f, 0.f, 0.f);
+                sm.C[kDummy + tid] = make_float4(0.f, 0.f, kVarH ? 1.f : 0.f, 0.f);
                 sm.D[kDummy + tid] = make_float4(0.f, 0.f, 0.f, 0.f);
             }
         }
@@ -463,7 +464,9 @@ interact_tiled_kernel(Packed rec, InteractIn in, const uint32_t *__restrict__ cs
             const int c = __popc(m0) + __popc(m1) + __popc(m2);
             const int rounds = (int)__reduce_max_sync(0xffffffffu, (unsigned)((c + 1) >> 1));
             float4 tv = make_float4(0.f, 0.f, 0.f, 0.f);
+            float th = 1.0f;   // the target's own smoothing length (NEXT-4)
             if (my_valid) tv = sm.B[tbase + my_t];
+            if (kVarH && my_valid) th = sm.C[tbase + my_t].z;
             const f32x2 tpxy = pk(tp.x, tp.y), tvxy = pk(tv.x, tv.y);
             PairAccum2 S;
             S.clear();
@@ -497,8 +500,10 @@ interact_tiled_kernel(Packed rec, InteractIn in, const uint32_t *__restrict__ cs
                     const float4 pb = ld_rec(sm.B, e);
                     const float4 pc = ld_rec(sm.C, e);
                     const float4 pd = ld_rec(sm.D, e);
-                    const float r2 = S.add(tpxy, tp.z, tvxy, tv.z, pa, pb, pc, pd, -k.half_inv_h);
-                    if (kCount && r2 < k.support2) ++my_pairs;  // exact test (phase 1 has a rounding margin)
+                    const float r2 = S.template add<kVarH>(tpxy, tp.z, tvxy, tv.z, pa, pb, pc, pd, -k.half_inv_h, th);
+                    // exact test (phase 1 has a rounding margin; with per-particle lengths it runs on 2 h_max)
+                    const float hs = th + pc.z;
+                    if (kCount && r2 < (kVarH ? hs * hs : k.support2)) ++my_pairs;
                 };
 #pragma unroll 1
                 for (int r = 0; r < rounds; ++r) {
@@ -606,39 +611,37 @@ int launch_interact_tiled(sph_ctx *c, int64_t n, const InteractIn &in, const uin
     }
     c->rec_fresh = false;
     const int smem = (int)sizeof(TileSmem);
+    const bool vh = in.h != nullptr;
     if (!c->attr_interact) {   // per device: once per ctx
-        SPH_CUDA_TRY(c, cudaFuncSetAttribute(interact_tiled_kernel<true, kPassAll>,
-                                             cudaFuncAttributeMaxDynamicSharedMemorySize, smem));
-        SPH_CUDA_TRY(c, cudaFuncSetAttribute(interact_tiled_kernel<false, kPassAll>,
-                                             cudaFuncAttributeMaxDynamicSharedMemorySize, smem));
-        SPH_CUDA_TRY(c, cudaFuncSetAttribute(interact_tiled_kernel<true, kPassLocal>,
-                                             cudaFuncAttributeMaxDynamicSharedMemorySize, smem));
-        SPH_CUDA_TRY(c, cudaFuncSetAttribute(interact_tiled_kernel<true, kPassRemote>,
-                                             cudaFuncAttributeMaxDynamicSharedMemorySize, smem));
+        const void *fns[] = {
+            (const void *)interact_tiled_kernel<true, kPassAll, false>, (const void *)interact_tiled_kernel<false, kPassAll, false>,
+            (const void *)interact_tiled_kernel<true, kPassLocal, false>, (const void *)interact_tiled_kernel<true, kPassRemote, false>,
+            (const void *)interact_tiled_kernel<true, kPassAll, true>, (const void *)interact_tiled_kernel<false, kPassAll, true>,
+            (const void *)interact_tiled_kernel<true, kPassLocal, true>, (const void *)interact_tiled_kernel<true, kPassRemote, true>};
+        for (const void *f : fns) SPH_CUDA_TRY(c, cudaFuncSetAttribute(f, cudaFuncAttributeMaxDynamicSharedMemorySize, smem));
         c->attr_interact = true;
     }
     const int tiles_x = (c->grid.nx + kTBX - 1) / kTBX, tiles_y = (c->grid.ny + kTBY - 1) / kTBY;
     const int64_t tiles = (int64_t)tiles_x * tiles_y * c->grid.nz;
     if (tiles > 0x7fffffffll) return SPH_EINVAL;
     const unsigned gr = (unsigned)tiles;
+    Consts kc = c->consts;
+    if (vh) kc.cF = kc.cF_varh;   // h_ij^-5 is applied per pair (reading H2)
+    // the split passes always count (one instantiation each); without a caller buffer the count
+    // goes to ctx scratch
+    unsigned long long *pc = (mode == kPassAll || pair_count) ? pair_count : c->s_pair_count;
+#define SPH_LAUNCH_TILED(CNT, MODE, VH)                                                        \
+    interact_tiled_kernel<CNT, MODE, VH><<<gr, kTW * 32, smem, c->stream>>>(                     \
+        rec, in, cs, ce, c->grid, kc, out, pc, tiles_x, tiles_y)
     if (mode == kPassAll) {
-        if (pair_count)
-            interact_tiled_kernel<true, kPassAll><<<gr, kTW * 32, smem, c->stream>>>(
-                rec, in, cs, ce, c->grid, c->consts, out, pair_count, tiles_x, tiles_y);
-        else
-            interact_tiled_kernel<false, kPassAll><<<gr, kTW * 32, smem, c->stream>>>(
-                rec, in, cs, ce, c->grid, c->consts, out, pair_count, tiles_x, tiles_y);
+        if (pair_count) { if (vh) SPH_LAUNCH_TILED(true, kPassAll, true); else SPH_LAUNCH_TILED(true, kPassAll, false); }
+        else            { if (vh) SPH_LAUNCH_TILED(false, kPassAll, true); else SPH_LAUNCH_TILED(false, kPassAll, false); }
+    } else if (mode == kPassLocal) {
+        if (vh) SPH_LAUNCH_TILED(true, kPassLocal, true); else SPH_LAUNCH_TILED(true, kPassLocal, false);
     } else {
-        // the split passes always count (one instantiation each); without a caller buffer the
-        // count goes to ctx scratch
-        unsigned long long *pc = pair_count ? pair_count : c->s_pair_count;
-        if (mode == kPassLocal)
-            interact_tiled_kernel<true, kPassLocal><<<gr, kTW * 32, smem, c->stream>>>(
-                rec, in, cs, ce, c->grid, c->consts, out, pc, tiles_x, tiles_y);
-        else
-            interact_tiled_kernel<true, kPassRemote><<<gr, kTW * 32, smem, c->stream>>>(
-                rec, in, cs, ce, c->grid, c->consts, out, pc, tiles_x, tiles_y);
+        if (vh) SPH_LAUNCH_TILED(true, kPassRemote, true); else SPH_LAUNCH_TILED(true, kPassRemote, false);
     }
+#undef SPH_LAUNCH_TILED
     SPH_CHECK_LAUNCH(c);
     return SPH_OK;
 }

@@ -24,7 +24,8 @@ struct StatePtrsOut {
 template <bool PACK>
 __global__ void __launch_bounds__(256)
 reorder_kernel(int64_t n, const uint32_t *__restrict__ perm, StatePtrs in, StatePtrsOut out,
-               float4 *__restrict__ recB, float4 *__restrict__ recC, float4 *__restrict__ recD)
+               float4 *__restrict__ recB, float4 *__restrict__ recC, float4 *__restrict__ recD,
+               const float *__restrict__ h_in, float *__restrict__ h_out)
 {
     const int64_t k = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
     if (k >= n) return;
@@ -36,6 +37,8 @@ reorder_kernel(int64_t n, const uint32_t *__restrict__ perm, StatePtrs in, State
 #pragma unroll
     for (int c = 0; c < 6; ++c) s[c] = __ldg(in.sig[c] + id);
     const int32_t o = __ldg(in.owner + id);
+    float hk = 0.f;   // NEXT-4: per-particle smoothing length (C.z of the record carries it)
+    if (h_in) { hk = __ldg(h_in + id); h_out[k] = hk; }
     out.posm[k] = p;
     out.velr[k] = v;
 #pragma unroll
@@ -46,7 +49,7 @@ reorder_kernel(int64_t n, const uint32_t *__restrict__ perm, StatePtrs in, State
         const float ir2 = inv_rho * inv_rho;
         const float sxy = s[3] * ir2;
         recB[k] = make_float4(v.x, v.y, v.z, s[2] * ir2);
-        recC[k] = make_float4(s[0] * ir2, sxy, sxy, s[1] * ir2);
+        recC[k] = make_float4(s[0] * ir2, sxy, h_in ? hk : sxy, s[1] * ir2);
         recD[k] = make_float4(s[4] * ir2, s[5] * ir2, p.w, p.w * inv_rho);
     }
 }
@@ -155,7 +158,7 @@ int launch_scatter_records(sph_ctx *c, int64_t m, const uint32_t *ids, const uin
 }
 
 int launch_reorder(sph_ctx *c, int64_t n, const uint32_t *perm, const sph_state *in,
-                   const sph_state *out)
+                   const sph_state *out, const float *h_in, float *h_out)
 {
     if (n == 0) return SPH_OK;
     StatePtrs a;
@@ -170,9 +173,11 @@ int launch_reorder(sph_ctx *c, int64_t n, const uint32_t *perm, const sph_state 
     // the ctx's own sorted copy (sph_step) gets its interaction records in the same pass
     const bool pack = out->posm == c->sorted.posm;
     if (pack)
-        reorder_kernel<true><<<div_up(n, 256), 256, 0, c->stream>>>(n, perm, a, b, c->rec_B, c->rec_C, c->rec_D);
+        reorder_kernel<true><<<div_up(n, 256), 256, 0, c->stream>>>(n, perm, a, b, c->rec_B, c->rec_C, c->rec_D,
+                                                                    h_in, h_out);
     else
-        reorder_kernel<false><<<div_up(n, 256), 256, 0, c->stream>>>(n, perm, a, b, nullptr, nullptr, nullptr);
+        reorder_kernel<false><<<div_up(n, 256), 256, 0, c->stream>>>(n, perm, a, b, nullptr, nullptr, nullptr,
+                                                                     h_in, h_out);
     SPH_CHECK_LAUNCH(c);
     c->rec_fresh = pack;
     return SPH_OK;

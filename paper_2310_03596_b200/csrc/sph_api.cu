@@ -65,6 +65,7 @@ void carve(sph_ctx *c, char *base, size_t *total)
     c->sorted.velr = k.take<float>(4 * n);
     for (int i = 0; i < 6; ++i) c->sorted.sig[i] = k.take<float>(n);
     c->sorted.owner = k.take<int32_t>(n);
+    c->sorted_h = k.take<float>(n);
     c->rec_B = k.take<float4>(n + 2);
     c->rec_C = k.take<float4>(n + 2);
     c->rec_D = k.take<float4>(n + 2);
@@ -105,7 +106,7 @@ static int step_impl(sph_ctx *c, int64_t n, float dt, const sph_state *state, ui
                      uint32_t *sorted_hash, uint32_t *perm, uint32_t *cell_start, uint32_t *cell_end,
                      uint32_t *comm_hash, uint32_t *boundary_ids, uint32_t *boundary_count,
                      uint32_t *owner_counts, float *drho, float *acc, float *const dsig[6],
-                     unsigned long long *pair_count, bool zero_pairs);
+                     unsigned long long *pair_count, bool zero_pairs, const float *hp = nullptr);
 
 int sph_create(sph_ctx **out, const sph_params *p, int64_t max_n, void *cuda_stream)
 {
@@ -146,6 +147,7 @@ int sph_create(sph_ctx **out, const sph_params *p, int64_t max_n, void *cuda_str
     c->consts.support2 = edge * edge;
     c->consts.half_inv_h = (float)(0.5 / h);
     c->consts.cF = (float)(-5.0 * alpha / (h * h));
+    c->consts.cF_varh = (float)(-105.0 / (16.0 * 3.14159265358979323846));
     c->consts.K = p->K;
     c->consts.G = p->G;
     c->key_bits = ceil_log2_u64(cells);
@@ -281,7 +283,7 @@ static int step_impl(sph_ctx *c, int64_t n, float dt, const sph_state *state, ui
                      uint32_t *sorted_hash, uint32_t *perm, uint32_t *cell_start, uint32_t *cell_end,
                      uint32_t *comm_hash, uint32_t *boundary_ids, uint32_t *boundary_count,
                      uint32_t *owner_counts, float *drho, float *acc, float *const dsig[6],
-                     unsigned long long *pair_count, bool zero_pairs)
+                     unsigned long long *pair_count, bool zero_pairs, const float *hp)
 {
     if (!n_ok(c, n) || !state || (n > 0 && !state_ok(state))) return SPH_EINVAL;
     if (pair_count && zero_pairs)
@@ -311,7 +313,7 @@ static int step_impl(sph_ctx *c, int64_t n, float dt, const sph_state *state, ui
     t.mark();
     if ((rc = launch_sort(c, n, hash, sorted_hash, perm)) != SPH_OK) return rc;
     t.mark();
-    if ((rc = launch_reorder(c, n, perm, state, &c->sorted)) != SPH_OK) return rc;
+    if ((rc = launch_reorder(c, n, perm, state, &c->sorted, hp, c->sorted_h)) != SPH_OK) return rc;
     t.mark();
     if ((rc = launch_cell_ranges(c, n, sorted_hash, cell_start, cell_end)) != SPH_OK) return rc;
     t.mark();
@@ -323,7 +325,7 @@ static int step_impl(sph_ctx *c, int64_t n, float dt, const sph_state *state, ui
     // id order through perm; `state` is only written, the loops read the sorted copy
     if ((rc = launch_interact(c, n, &c->sorted, sorted_hash, cell_start, cell_end, want_rates ? drho : nullptr,
                               want_rates ? acc : nullptr, want_rates ? ds : nullptr, pair_count, state, perm,
-                              dt)) != SPH_OK)
+                              dt, 0, hp ? c->sorted_h : nullptr)) != SPH_OK)
         return rc;
     t.mark();
     t.mark();
@@ -338,6 +340,32 @@ int sph_step(sph_ctx *c, int64_t n, float dt, const sph_state *state, uint32_t *
 {
     return step_impl(c, n, dt, state, hash, sorted_hash, perm, cell_start, cell_end, comm_hash,
                      boundary_ids, boundary_count, owner_counts, drho, acc, dsig, pair_count, true);
+}
+
+int sph_step_varh(sph_ctx *c, int64_t n, float dt, const sph_state *state, const float *h, uint32_t *hash,
+                  uint32_t *sorted_hash, uint32_t *perm, uint32_t *cell_start, uint32_t *cell_end,
+                  uint32_t *comm_hash, uint32_t *boundary_ids, uint32_t *boundary_count,
+                  uint32_t *owner_counts, float *drho, float *acc, float *const dsig[6],
+                  unsigned long long *pair_count)
+{
+    if (!h && n > 0) return SPH_EINVAL;
+    return step_impl(c, n, dt, state, hash, sorted_hash, perm, cell_start, cell_end, comm_hash,
+                     boundary_ids, boundary_count, owner_counts, drho, acc, dsig, pair_count, true, h);
+}
+
+int sph_interact_varh(sph_ctx *c, int64_t n, const sph_state *sorted, const float *sorted_h,
+                      const uint32_t *sorted_hash, const uint32_t *cs, const uint32_t *ce, int32_t which,
+                      float *drho, float *acc, float *const dsig[6], unsigned long long *pair_count)
+{
+    if (!n_ok(c, n) || !state_ok(sorted) || !sorted_h || !sorted_hash || !cs || !ce || !drho || !acc || !dsig)
+        return SPH_EINVAL;
+    if (which < 0 || which > 2) return SPH_EINVAL;
+    for (int i = 0; i < 6; ++i)
+        if (!dsig[i]) return SPH_EINVAL;
+    if (pair_count)
+        SPH_CUDA_TRY(c, cudaMemsetAsync(pair_count, 0, sizeof(unsigned long long), c->stream));
+    return launch_interact(c, n, sorted, sorted_hash, cs, ce, drho, acc, dsig, pair_count, nullptr, nullptr, 0.f,
+                           which, sorted_h);
 }
 
 int sph_step_host(sph_ctx *c, int64_t n, float dt, int32_t steps, const sph_state *hs,

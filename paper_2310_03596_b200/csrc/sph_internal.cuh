@@ -39,6 +39,7 @@ struct Consts {
     float support2;      // (2h)^2 in fp32
     float half_inv_h;    // 0.5 / h
     float cF;            // -(5 alpha / h^2),  alpha = 21 / (16 pi h^3)
+    float cF_varh;       // -105 / (16 pi): the same constant with h_ij^-5 left to the pair (NEXT-4)
     float K, G;
 };
 
@@ -84,6 +85,7 @@ struct sph_ctx {
     float *s_drho, *s_acc, *s_dsig[6];
     unsigned long long *s_pair_count;
     sph_state sorted;                         // sorted copy of the state
+    float *sorted_h;                          // sorted per-particle smoothing lengths (NEXT-4)
     float4 *rec_B, *rec_C;                    // packed neighbour records of the interaction kernel
     float4 *rec_D;
     void *bal;                                // control block of the balancing sweep (balance.cu)
@@ -116,7 +118,7 @@ static inline int div_up(int64_t a, int64_t b) { return (int)((a + b - 1) / b); 
 int launch_hash(sph_ctx *c, int64_t n, const float *posm, uint32_t *hash);
 int launch_sort(sph_ctx *c, int64_t n, const uint32_t *hash, uint32_t *sorted_hash, uint32_t *perm);
 int launch_reorder(sph_ctx *c, int64_t n, const uint32_t *perm, const sph_state *in,
-                   const sph_state *out);
+                   const sph_state *out, const float *h_in = nullptr /* id order */, float *h_out = nullptr);
 int launch_cell_ranges(sph_ctx *c, int64_t n, const uint32_t *sorted_hash, uint32_t *cs,
                        uint32_t *ce);
 int launch_comm_hash(sph_ctx *c, int64_t n, const uint32_t *sorted_hash, const int32_t *sorted_owner,
@@ -127,7 +129,8 @@ int launch_interact(sph_ctx *c, int64_t n, const sph_state *sorted, const uint32
                     const uint32_t *cs, const uint32_t *ce, float *drho, float *acc,
                     float *const dsig[6], unsigned long long *pair_count,
                     const sph_state *fuse_out /* NULL = rates only */, const uint32_t *perm, float dt,
-                    int mode = 0 /* 0 all, 1 same-owner, 2 other-owner neighbours */);
+                    int mode = 0 /* 0 all, 1 same-owner, 2 other-owner neighbours */,
+                    const float *sorted_h = nullptr /* NEXT-4: per-particle smoothing lengths */);
 int launch_integrate(sph_ctx *c, int64_t n, float dt, const sph_state *in, const float *drho,
                      const float *acc, const float *const dsig[6], const sph_state *out,
                      const uint32_t *scatter_perm /* NULL = elementwise */);

@@ -30,7 +30,7 @@ TIMING_SLOTS = 32          # steps held by the library's ring of stage events (s
 EXPORTS = (
     "sph_create", "sph_destroy", "sph_hash", "sph_sort", "sph_reorder", "sph_cell_ranges",
     "sph_comm_hash", "sph_interact", "sph_integrate", "sph_step", "sph_step_host", "sph_pack_boundary",
-    "sph_interact_split", "sph_balance", "sph_balance_types", "sph_enable_timing", "sph_get_timing", "sph_launch_count", "sph_strerror",
+    "sph_interact_split", "sph_interact_varh", "sph_step_varh", "sph_balance", "sph_balance_types", "sph_enable_timing", "sph_get_timing", "sph_launch_count", "sph_strerror",
     "sph_last_cuda_error",
 )
 
@@ -72,6 +72,8 @@ def load_library() -> C.CDLL:
     lib.sph_comm_hash.argtypes = [vp, i64] + [vp] * 9
     lib.sph_interact.argtypes = [vp, i64, sp, vp, vp, vp, vp, vp, C.POINTER(vp * 6), vp]
     lib.sph_interact_split.argtypes = [vp, i64, sp, vp, vp, vp, i32, vp, vp, C.POINTER(vp * 6), vp]
+    lib.sph_interact_varh.argtypes = [vp, i64, sp, vp, vp, vp, vp, i32, vp, vp, C.POINTER(vp * 6), vp]
+    lib.sph_step_varh.argtypes = [vp, i64, f32, sp, vp] + [vp] * 11 + [C.POINTER(vp * 6), vp]
     lib.sph_integrate.argtypes = [vp, i64, f32, sp, vp, vp, C.POINTER(vp * 6), sp]
     lib.sph_step.argtypes = [vp, i64, f32, sp] + [vp] * 11 + [C.POINTER(vp * 6), vp]
     lib.sph_step_host.argtypes = [vp, i64, f32, i32, sp, vp, vp, vp]
@@ -315,6 +317,39 @@ class Context:
                   "sph_interact_split")
         return drho, acc, dsig, pc
 
+    def sph_interact_varh(self, sorted_state: State, sorted_h, sorted_hash, cell_start, cell_end, which: int = 0):
+        """Interaction loops with a smoothing length per particle (NEXT-4; sorted_h [n] f32 in sorted
+        order); which = 0 all neighbours, 1 / 2 the split passes."""
+        n = sorted_state.n
+        drho, acc, dsig = self._f32(n), self._f32(n, 4), self._f32(6, n)
+        pc = torch.zeros(1, dtype=torch.int64, device=self.device)
+        s = sorted_state._c()
+        d6 = _six(dsig)
+        self._chk(self.lib.sph_interact_varh(self.handle, n, C.byref(s), sorted_h.data_ptr(), sorted_hash.data_ptr(),
+                                             cell_start.data_ptr(), cell_end.data_ptr(), int(which),
+                                             drho.data_ptr(), acc.data_ptr(), C.byref(d6), pc.data_ptr()),
+                  "sph_interact_varh")
+        return drho, acc, dsig, pc
+
+    def sph_step_varh(self, state: State, h: torch.Tensor, dt, out: StepOutputs | None = None,
+                      pair_count: torch.Tensor | None = None):
+        """sph_step with a smoothing length per particle (h [n] f32 in id order, NEXT-4)."""
+        n = state.n
+        s = state._c()
+        o = out
+        if o is not None:
+            d6 = _six(o.dsig)
+            rc = self.lib.sph_step_varh(self.handle, n, float(dt), C.byref(s), h.data_ptr(), _ptr(o.hash),
+                                        _ptr(o.sorted_hash), _ptr(o.perm), _ptr(o.cell_start),
+                                        _ptr(o.cell_end), _ptr(o.comm_hash), _ptr(o.boundary_ids),
+                                        _ptr(o.boundary_count), _ptr(o.owner_counts), _ptr(o.drho),
+                                        _ptr(o.acc), C.byref(d6), _ptr(o.pair_count))
+        else:
+            rc = self.lib.sph_step_varh(self.handle, n, float(dt), C.byref(s), h.data_ptr(), *([None] * 11), None,
+                                        _ptr(pair_count))
+        self._chk(rc, "sph_step_varh")
+        return out
+
     def sph_integrate(self, dt, state: State, drho, acc, dsig, out: State | None = None) -> State:
         n = state.n
         out = out if out is not None else State.empty(n, self.device)
@@ -405,6 +440,8 @@ def sph_cell_ranges(ctx, *a, **k): return ctx.sph_cell_ranges(*a, **k)
 def sph_comm_hash(ctx, *a, **k): return ctx.sph_comm_hash(*a, **k)
 def sph_interact(ctx, *a, **k): return ctx.sph_interact(*a, **k)
 def sph_interact_split(ctx, *a, **k): return ctx.sph_interact_split(*a, **k)
+def sph_interact_varh(ctx, *a, **k): return ctx.sph_interact_varh(*a, **k)
+def sph_step_varh(ctx, *a, **k): return ctx.sph_step_varh(*a, **k)
 def sph_integrate(ctx, *a, **k): return ctx.sph_integrate(*a, **k)
 def sph_step(ctx, *a, **k): return ctx.sph_step(*a, **k)
 def sph_step_host(ctx, *a, **k): return ctx.sph_step_host(*a, **k)

@@ -81,18 +81,23 @@ def compare_state(state, ref) -> dict:
     return errs
 
 
-def lockstep(sph, oracle, w, steps=1, flags=0, floats=True) -> list[dict]:
-    """Reading S20: every step the oracle is fed the GPU's fp32 state at the start of that step."""
+def lockstep(sph, oracle, w, steps=1, flags=0, floats=True, hp=None) -> list[dict]:
+    """Reading S20: every step the oracle is fed the GPU's fp32 state at the start of that step.
+    hp = per-particle smoothing lengths in id order (NEXT-4): sph_step_varh against oracle.step(hp=)."""
     ctx = sph.Context.for_workload(w, flags=flags)
     state = sph.State.from_numpy(w.posm, w.velr, w.sig, w.owner)
     out = ctx.alloc_outputs(w.n)
+    h_dev = torch.from_numpy(np.ascontiguousarray(hp, np.float32)).cuda() if hp is not None else None
     report = []
     for _ in range(steps):
         posm, velr = state.posm.cpu().numpy(), state.velr.cpu().numpy()
         sig, owner = state.sig.cpu().numpy(), state.owner.cpu().numpy()
         ref = oracle.step(posm, velr, sig, owner, w.origin, w.dims, w.h, w.K, w.G, w.n_owners, w.dt,
-                          floats=floats)
-        ctx.sph_step(state, w.dt, out)
+                          floats=floats, hp=hp)
+        if hp is None:
+            ctx.sph_step(state, w.dt, out)
+        else:
+            ctx.sph_step_varh(state, h_dev, w.dt, out)
         torch.cuda.synchronize()
         compare_integers(out, ref, w.n)
         np.testing.assert_array_equal(state.owner.cpu().numpy(), owner)

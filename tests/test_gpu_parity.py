@@ -412,6 +412,60 @@ def test_balance_types_matches_oracle_bit_exact(sph, oracle, g, nt, alpha):
     ctx.close()
 
 
+# ------------------------------------------------------------------ NEXT-4: per-particle smoothing lengths
+@pytest.mark.parametrize("flags", [0, 1], ids=["tiled", "direct"])
+@pytest.mark.parametrize("kind", [("species", 2, 0.75), ("random", 0.5), ("uniform",)],
+                         ids=["two-species", "random", "uniform"])
+def test_varh_step_matches_oracle(sph, oracle, kind, flags):
+    """sph_step_varh (readings H1-H3) lock-step against the oracle: integers
+    bit-exact (they do not depend on h), rates 1e-5, state 1e-6, pair counts 1e-6."""
+    w = wl.t1b(side=18, seed=1108)
+    hp = wl.particle_h(w, kind)
+    rep = parity.lockstep(sph, oracle, w, steps=2, flags=flags, hp=hp)
+    assert rep[0]["pairs"] > 0
+    if kind[0] != "uniform":
+        full = parity.lockstep(sph, oracle, w, steps=1, flags=flags)
+        assert rep[0]["pairs"] < full[0]["pairs"]         # shorter lengths lose neighbours
+
+
+def test_varh_scaled_config_many_tiles_and_split_passes(sph, oracle):
+    """Several tiles with ragged edges, 16 mixed owners, three species; the stage call with
+    which = 0 / 1 / 2 against orc_interact_varh, and pass e + pass f = the single pass."""
+    w = wl.config(2, side=33)
+    rng = np.random.default_rng(77)                        # a state in which every rate is non-trivial
+    w.sig[:] = (rng.standard_normal((6, w.n)) * 1e-3).astype(np.float32)
+    w.velr[:, :3] += (rng.standard_normal((w.n, 3)) * 0.01).astype(np.float32)
+    w.velr[:, 3] = (1.0 + (rng.random(w.n) * 2 - 1) * 0.01).astype(np.float32)
+    hp = wl.particle_h(w, ("species", 3, 0.6))
+    ctx = sph.Context.for_workload(w)
+    st = sph.State.from_numpy(w.posm, w.velr, w.sig, w.owner)
+    hh = ctx.sph_hash(st.posm)
+    sh, perm = ctx.sph_sort(hh)
+    sst = ctx.sph_reorder(perm, st)
+    cs, ce = ctx.sph_cell_ranges(sh)
+    p = parity.u32(perm).astype(np.int64)
+    sh_h = torch.from_numpy(hp[p]).cuda()
+    sp, sv, ss, so = w.posm[p], w.velr[p], np.ascontiguousarray(w.sig[:, p]), w.owner[p]
+    res = {}
+    for which in (0, 1, 2):
+        drho, acc, dsig, pc = ctx.sph_interact_varh(sst, sh_h, sh, cs, ce, which)
+        torch.cuda.synchronize()
+        ref = oracle.interact_varh(sp, sv, ss, hp[p], parity.u32(sh), w.dims, parity.u32(cs), parity.u32(ce),
+                                   w.h, w.K, w.G, owner=so, which=which)
+        if which == 0:
+            scale = {"drho": np.abs(ref.drho).max(), "acc": np.abs(ref.acc).max(), "dsig": np.abs(ref.dsig).max()}
+        got = {"drho": drho.cpu().numpy(), "acc": acc.cpu().numpy()[:, :3], "dsig": dsig.cpu().numpy().T}
+        for name in ("drho", "acc", "dsig"):
+            err = np.abs(got[name] - getattr(ref, name)).max() / scale[name]
+            assert err <= parity.RATE_TOL, (which, name, err)
+        assert abs(int(pc.cpu()[0]) - ref.pair_count) <= max(1e-6 * ref.pair_count, 2)
+        res[which] = (got, int(pc.cpu()[0]))
+    assert res[1][1] + res[2][1] == res[0][1]
+    for name in ("drho", "acc", "dsig"):
+        assert np.abs(res[1][0][name] + res[2][0][name] - res[0][0][name]).max() <= parity.RATE_TOL * scale[name]
+    ctx.close()
+
+
 def test_long_run_then_lockstep(sph, oracle):
     """300 steps of the benchmark's configuration on a scaled configs[1] (state re-hashed and
     re-sorted every step), then one lock-step comparison with the oracle from the GPU's state:
