@@ -66,10 +66,13 @@ bal_sums_kernel(int64_t n, const float4 *__restrict__ posm, const int32_t *__res
         if ((&s_cnt[0][0])[i]) atomicAdd(&ctl->cnt[0][0] + i, (&s_cnt[0][0])[i]);
 }
 
-// one thread: centres of gravity of the pair, validity, cleared histograms
-__global__ void bal_pair_begin_kernel(BalCtl *ctl, int A, int B, int T, int typed, double alpha)
+// one block: centres of gravity of the pair, validity, cleared histograms and look-back words
+__global__ void bal_pair_begin_kernel(BalCtl *ctl, int A, int B, int T, int typed, double alpha,
+                                      uint32_t *status, int64_t n_status, uint32_t *ticket)
 {
     for (int i = threadIdx.x; i < 2 * kBalBins; i += blockDim.x) (&ctl->hist[0][0])[i] = 0;
+    for (int64_t i = threadIdx.x; i < n_status; i += blockDim.x) status[i] = 0;   // look-back words of pass 2
+    if (threadIdx.x == 0) *ticket = 0;
     if (threadIdx.x != 0) return;
     const unsigned long long ca = ctl->cnt[A][T], cb = ctl->cnt[B][T];
     int valid = ca != 0 && cb != 0;   // B5 / B10
@@ -111,26 +114,86 @@ __device__ __forceinline__ int32_t balance_hash(const float4 &p, const double *o
     return (int32_t)hv;
 }
 
+// Per pair the particles are visited TWICE, both times as a dense stream:
+//   pass 1 (bal_hash_kernel): owner labels in, balancing hash of the pair's particles out, plus a
+//     dense 16-bit code per particle (0 = takes no part or hash 0; else side bit 14 | hash), plus
+//     the two 1024-bin histograms;
+//   pass 2 (bal_swap_kernel): codes in; the ties at the threshold hash are ranked by id with a
+//     decoupled look-back over the tiles (two status words per tile, one per side) INSIDE the
+//     pass, and the labels of the selected particles are flipped at once.
+// (The first version ran seven full-length passes per pair: hash, tie indicators, two separate
+// scans reading and writing 4 B per particle each, swap: 1.4-1.9 ms per pair at 64 M particles.)
+constexpr int kBalThreads = 256;
+constexpr int kBalItems = 32;
+constexpr int kBalTile = kBalThreads * kBalItems;   // ids per tile of pass 2
+
+__device__ __forceinline__ uint16_t bal_code(int32_t hv, int side)
+{
+    return hv > 0 ? (uint16_t)((side ? 0x4000 : 0) | hv) : (uint16_t)0;
+}
+
 __global__ void __launch_bounds__(256)
 bal_hash_kernel(int64_t n, const float4 *__restrict__ posm, const int32_t *__restrict__ owner,
                 const int32_t *__restrict__ ptype, BalCtl *ctl, int A, int B, int T, int hmax,
-                int32_t *__restrict__ bal_hash)
+                int32_t *__restrict__ bal_hash, uint16_t *__restrict__ code)
 {
     __shared__ uint32_t s_hist[2][kBalBins];
     for (int i = threadIdx.x; i < 2 * kBalBins; i += blockDim.x) (&s_hist[0][0])[i] = 0;
     __syncthreads();
     if (ctl->valid) {
-        for (int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; i < n;
-             i += (int64_t)gridDim.x * blockDim.x) {
-            const int o = owner[i];
-            if (o != A && o != B) continue;
-            if (ptype && ptype[i] != T) continue;
-            const float4 p = posm[i];
+        const double cgA[3] = {ctl->cgA[0], ctl->cgA[1], ctl->cgA[2]};
+        const double cgB[3] = {ctl->cgB[0], ctl->cgB[1], ctl->cgB[2]};
+        // hash = hmax is by far the most frequent positive value (every particle beyond the other
+        // Cg): those are counted per thread and warp-reduced instead of hammering one shared bin
+        uint32_t n_max = 0;   // low half: side A, high half: side B
+        auto member = [&](int o, int t) -> bool { return (o == A || o == B) && (!ptype || t == T); };
+        auto hash_of = [&](int64_t i, int o, const float4 &p) -> uint16_t {
             const int side = o == A ? 0 : 1;
-            const int32_t hv = side == 0 ? balance_hash(p, ctl->cgA, ctl->cgB, hmax)
-                                         : balance_hash(p, ctl->cgB, ctl->cgA, hmax);
-            bal_hash[i] = hv;
-            if (hv > 0) atomicAdd(&s_hist[side][hv], 1u);
+            const int32_t hv = side == 0 ? balance_hash(p, cgA, cgB, hmax) : balance_hash(p, cgB, cgA, hmax);
+            if (bal_hash) bal_hash[i] = hv;   // optional product: a 4-byte scatter per member
+            if (hv == hmax) n_max += side ? 0x10000u : 1u;
+            else if (hv > 0) atomicAdd(&s_hist[side][hv], 1u);
+            return bal_code(hv, side);
+        };
+        // eight particles per thread and iteration: two 128-bit owner loads, then the position
+        // gathers of all members in flight together, one 128-bit code store
+        const bool vec = ((reinterpret_cast<uintptr_t>(owner) | (ptype ? reinterpret_cast<uintptr_t>(ptype) : 0)) & 15) == 0 &&
+                         (reinterpret_cast<uintptr_t>(code) & 15) == 0;
+        const int64_t n8 = vec ? (n >> 3) : 0;
+        for (int64_t g = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; g < n8; g += (int64_t)gridDim.x * blockDim.x) {
+            const int4 oa = __ldcs(reinterpret_cast<const int4 *>(owner) + 2 * g);
+            const int4 ob = __ldcs(reinterpret_cast<const int4 *>(owner) + 2 * g + 1);
+            int4 ta = make_int4(0, 0, 0, 0), tb = ta;
+            if (ptype) {
+                ta = __ldcs(reinterpret_cast<const int4 *>(ptype) + 2 * g);
+                tb = __ldcs(reinterpret_cast<const int4 *>(ptype) + 2 * g + 1);
+            }
+            const int o[8] = {oa.x, oa.y, oa.z, oa.w, ob.x, ob.y, ob.z, ob.w};
+            const int t[8] = {ta.x, ta.y, ta.z, ta.w, tb.x, tb.y, tb.z, tb.w};
+            const int64_t i = g << 3;
+            float4 p[8];
+            bool m[8];
+#pragma unroll
+            for (int j = 0; j < 8; ++j) {
+                m[j] = member(o[j], t[j]);
+                p[j] = m[j] ? __ldg(posm + i + j) : make_float4(0.f, 0.f, 0.f, 0.f);
+            }
+            uint32_t c[8];
+#pragma unroll
+            for (int j = 0; j < 8; ++j) c[j] = m[j] ? hash_of(i + j, o[j], p[j]) : 0u;
+            __stcs(reinterpret_cast<uint4 *>(code) + g,
+                   make_uint4(c[0] | (c[1] << 16), c[2] | (c[3] << 16), c[4] | (c[5] << 16), c[6] | (c[7] << 16)));
+        }
+        for (int64_t i = (n8 << 3) + (int64_t)blockIdx.x * blockDim.x + threadIdx.x; i < n;
+             i += (int64_t)gridDim.x * blockDim.x) {
+            const int o = owner[i], t = ptype ? ptype[i] : 0;
+            code[i] = member(o, t) ? hash_of(i, o, __ldg(posm + i)) : (uint16_t)0;
+        }
+        // (a thread sees at most n / (grid x 256 x 4) x 4 < 2^16 particles per side for n < 2^30)
+        const uint32_t wa = __reduce_add_sync(0xffffffffu, n_max & 0xFFFFu), wb = __reduce_add_sync(0xffffffffu, n_max >> 16);
+        if ((threadIdx.x & 31) == 0) {
+            if (wa) atomicAdd(&s_hist[0][hmax], wa);
+            if (wb) atomicAdd(&s_hist[1][hmax], wb);
         }
     }
     __syncthreads();
@@ -186,50 +249,111 @@ __global__ void __launch_bounds__(kBalBins) bal_pair_select_kernel(BalCtl *ctl, 
     if (j == 0) ctl->swapped += m;
 }
 
-// indicator arrays of the threshold ties (their exclusive scans rank the ties by id)
-__global__ void __launch_bounds__(256)
-bal_ties_kernel(int64_t n, const int32_t *__restrict__ owner, const int32_t *__restrict__ ptype,
-                const int32_t *__restrict__ bal_hash, const BalCtl *ctl, int A, int B, int T,
-                uint32_t *__restrict__ tieA, uint32_t *__restrict__ tieB)
-{
-    const int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
-    if (i >= n) return;
-    uint32_t a = 0, b = 0;
-    if (ctl->valid) {
-        const int o = owner[i];
-        const bool mine = !ptype || ptype[i] == T;
-        if (mine && o == A) a = (uint32_t)bal_hash[i] == ctl->thrA;
-        else if (mine && o == B) b = (uint32_t)bal_hash[i] == ctl->thrB;
-    }
-    tieA[i] = a;
-    tieB[i] = b;
-}
-
-__global__ void __launch_bounds__(256)
+// Pass 2: one tile of kBalTile consecutive ids per block (dynamic ticket).  The ties at the
+// threshold hash of each side are ranked by id: block scan of the per-thread tie counts, then a
+// decoupled look-back over the preceding tiles (warp 0: side A, warp 1: side B); a particle moves
+// if its hash is above the threshold, or equal to it with rank < quota (reading B6).
+__global__ void __launch_bounds__(kBalThreads)
 bal_swap_kernel(int64_t n, const float4 *__restrict__ posm, int32_t *__restrict__ owner,
-                const int32_t *__restrict__ ptype, const int32_t *__restrict__ bal_hash, BalCtl *ctl, int A,
-                int B, int T, const uint32_t *__restrict__ rankA, const uint32_t *__restrict__ rankB)
+                const uint16_t *__restrict__ code, BalCtl *ctl, int A, int B, int T, uint32_t *statusA,
+                uint32_t *statusB, uint32_t *ticket)
 {
     // D = (coordinates leaving A) - (coordinates leaving B): sum[A] -= D, sum[B] += D.  Exact
     // integer sums, so the order of the block and grid reductions does not matter.
     __shared__ long long s_d[3];
-    if (threadIdx.x < 3) s_d[threadIdx.x] = 0;
+    __shared__ uint32_t s_warp[kBalThreads / 32];
+    __shared__ uint32_t s_tile, s_excl[2];
+    if (!ctl->valid) return;   // uniform over the grid: nothing to swap for this pair
+    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+    if (tid == 0) s_tile = atomicAdd(ticket, 1u);
+    if (tid < 3) s_d[tid] = 0;
     __syncthreads();
-    if (!ctl->valid) return;   // uniform over the grid
-    const int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
-    long long f[3] = {0, 0, 0};
-    if (i < n) {
-        const int o = owner[i];
-        if ((o == A || o == B) && (!ptype || ptype[i] == T)) {
-            const uint32_t hv = (uint32_t)bal_hash[i];
-            const uint32_t thr = o == A ? ctl->thrA : ctl->thrB, quota = o == A ? ctl->quotaA : ctl->quotaB;
-            const uint32_t rank = o == A ? rankA[i] : rankB[i];
-            if (hv > 0 && (hv > thr || (hv == thr && rank < quota))) {
-                owner[i] = o == A ? B : A;
-                const float4 p = posm[i];
-                const long long sgn = o == A ? 1 : -1;
-                f[0] = sgn * fixed16(p.x); f[1] = sgn * fixed16(p.y); f[2] = sgn * fixed16(p.z);
+    const uint32_t tile = s_tile;
+    const int64_t base = (int64_t)tile * kBalTile + (int64_t)tid * kBalItems;
+    const uint32_t thrA = ctl->thrA, thrB = ctl->thrB, quotaA = ctl->quotaA, quotaB = ctl->quotaB;
+    uint16_t c[kBalItems];
+    if (base + kBalItems <= n && (reinterpret_cast<uintptr_t>(code) & 15) == 0) {
+#pragma unroll
+        for (int q = 0; q < kBalItems / 8; ++q) {
+            const uint4 x = __ldcs(reinterpret_cast<const uint4 *>(code + base) + q);
+            c[8 * q] = (uint16_t)x.x; c[8 * q + 1] = (uint16_t)(x.x >> 16);
+            c[8 * q + 2] = (uint16_t)x.y; c[8 * q + 3] = (uint16_t)(x.y >> 16);
+            c[8 * q + 4] = (uint16_t)x.z; c[8 * q + 5] = (uint16_t)(x.z >> 16);
+            c[8 * q + 6] = (uint16_t)x.w; c[8 * q + 7] = (uint16_t)(x.w >> 16);
+        }
+    } else {
+#pragma unroll
+        for (int j = 0; j < kBalItems; ++j) c[j] = (base + j < n) ? code[base + j] : (uint16_t)0;
+    }
+    // ties of this thread: side A in the low half, side B in the high half (each <= 16)
+    uint32_t ties = 0;
+#pragma unroll
+    for (int j = 0; j < kBalItems; ++j) {
+        const uint32_t hv = c[j] & 0x3FFFu;
+        const bool sideB = c[j] & 0x4000u;
+        if (c[j] && hv == (sideB ? thrB : thrA)) ties += sideB ? 0x10000u : 1u;
+    }
+    uint32_t inc = ties;   // block scan (totals <= 4096 per side: 16 bits each are enough)
+#pragma unroll
+    for (int o = 1; o < 32; o <<= 1) {
+        const uint32_t x = __shfl_up_sync(0xffffffffu, inc, o);
+        if (lane >= o) inc += x;
+    }
+    if (lane == 31) s_warp[warp] = inc;
+    __syncthreads();
+    uint32_t add = 0, tile_total = 0;
+#pragma unroll
+    for (int i = 0; i < kBalThreads / 32; ++i) {
+        const uint32_t w = s_warp[i];
+        add += (i < warp) ? w : 0u;
+        tile_total += w;
+    }
+    if (warp < 2) {
+        // warp-parallel decoupled look-back (as in scan_exclusive_kernel), one side per warp
+        uint32_t *status = warp == 0 ? statusA : statusB;
+        const uint32_t mine = warp == 0 ? (tile_total & 0xFFFFu) : (tile_total >> 16);
+        if (lane == 0) st_volatile_u32(status + tile, (tile == 0 ? kFlagPrefix : kFlagAgg) | mine);
+        uint32_t excl = 0;
+        if (tile > 0) {
+            int64_t t0 = (int64_t)tile - 1;
+            while (true) {
+                const int64_t t = t0 - lane;
+                const uint32_t s = t >= 0 ? ld_volatile_u32(status + t) : kFlagPrefix;
+                const uint32_t f = s & kFlagMask;
+                const uint32_t pref = __ballot_sync(0xffffffffu, f == kFlagPrefix);
+                const uint32_t unpub = __ballot_sync(0xffffffffu, f == 0);
+                const int fp = pref ? __ffs(pref) - 1 : 31;
+                const uint32_t need = 0xffffffffu >> (31 - fp);
+                if (unpub & need) continue;
+                excl += __reduce_add_sync(0xffffffffu, lane <= fp ? (s & kValueMask) : 0u);
+                if (pref) break;
+                t0 -= 32;
             }
+            if (lane == 0) st_volatile_u32(status + tile, kFlagPrefix | (excl + mine));
+        }
+        if (lane == 0) s_excl[warp] = excl;
+    }
+    __syncthreads();
+    const uint32_t before = add + (inc - ties);
+    uint32_t rankA = s_excl[0] + (before & 0xFFFFu), rankB = s_excl[1] + (before >> 16);
+    long long f[3] = {0, 0, 0};
+#pragma unroll
+    for (int j = 0; j < kBalItems; ++j) {
+        if (!c[j]) continue;
+        const uint32_t hv = c[j] & 0x3FFFu;
+        const bool sideB = c[j] & 0x4000u;
+        const uint32_t thr = sideB ? thrB : thrA;
+        bool move = hv > thr;
+        if (hv == thr) {
+            move = sideB ? rankB < quotaB : rankA < quotaA;
+            if (sideB) ++rankB; else ++rankA;
+        }
+        if (move) {
+            const int64_t i = base + j;
+            owner[i] = sideB ? A : B;
+            const float4 p = __ldg(posm + i);
+            const long long sgn = sideB ? -1 : 1;
+            f[0] += sgn * fixed16(p.x); f[1] += sgn * fixed16(p.y); f[2] += sgn * fixed16(p.z);
         }
     }
 #pragma unroll
@@ -237,13 +361,13 @@ bal_swap_kernel(int64_t n, const float4 *__restrict__ posm, int32_t *__restrict_
         long long v = f[a];
 #pragma unroll
         for (int o = 16; o > 0; o >>= 1) v += __shfl_xor_sync(0xffffffffu, v, o);
-        if ((threadIdx.x & 31) == 0 && v) atomicAdd(reinterpret_cast<unsigned long long *>(&s_d[a]), (unsigned long long)v);
+        if (lane == 0 && v) atomicAdd(reinterpret_cast<unsigned long long *>(&s_d[a]), (unsigned long long)v);
     }
     __syncthreads();
-    if (threadIdx.x < 3 && s_d[threadIdx.x]) {
-        const long long d = s_d[threadIdx.x];
-        atomicAdd(reinterpret_cast<unsigned long long *>(&ctl->sum[A][T][threadIdx.x]), (unsigned long long)(-d));
-        atomicAdd(reinterpret_cast<unsigned long long *>(&ctl->sum[B][T][threadIdx.x]), (unsigned long long)d);
+    if (tid < 3 && s_d[tid]) {
+        const long long d = s_d[tid];
+        atomicAdd(reinterpret_cast<unsigned long long *>(&ctl->sum[A][T][tid]), (unsigned long long)(-d));
+        atomicAdd(reinterpret_cast<unsigned long long *>(&ctl->sum[B][T][tid]), (unsigned long long)d);
     }
 }
 
@@ -259,8 +383,11 @@ int launch_balance(sph_ctx *c, int64_t n, const float *posm, int32_t *owner, con
     // sweep per type with the biased Cg' of PAPER.md:56
     BalCtl *ctl = reinterpret_cast<BalCtl *>(c->bal);
     const float4 *p4 = reinterpret_cast<const float4 *>(posm);
-    int32_t *bh = bal_hash ? bal_hash : reinterpret_cast<int32_t *>(c->s_hash);
-    uint32_t *tieA = c->alt_keys, *tieB = c->alt_vals, *rankA = c->s_sorted_hash, *rankB = c->s_perm;
+    int32_t *bh = bal_hash;   // NULL: the hashes are not stored (pass 2 works on the 16-bit codes)
+    uint16_t *code = reinterpret_cast<uint16_t *>(c->alt_keys);          // scratch (stream-ordered)
+    const int64_t tiles = (n + kBalTile - 1) / kBalTile;
+    uint32_t *statusA = c->alt_vals, *statusB = c->alt_vals + tiles;     // tiles <= n / 2
+    uint32_t *ticket = c->tile_counter + kMaxPasses;
     SPH_CUDA_TRY(c, cudaMemsetAsync(ctl, 0, sizeof(BalCtl), c->stream));
     if (bal_hash) SPH_CUDA_TRY(c, cudaMemsetAsync(bal_hash, 0, sizeof(int32_t) * (size_t)n, c->stream));
     const int G = c->params.n_owners, NT = ptype ? n_types : 1, typed = ptype != nullptr;
@@ -271,20 +398,15 @@ int launch_balance(sph_ctx *c, int64_t n, const float *posm, int32_t *owner, con
         for (int T = 0; T < NT; ++T)
             for (int A = 0; A < G; ++A)
                 for (int B = A + 1; B < G; ++B) {
-                    bal_pair_begin_kernel<<<1, 256, 0, c->stream>>>(ctl, A, B, T, typed, alpha);
+                    bal_pair_begin_kernel<<<1, 256, 0, c->stream>>>(ctl, A, B, T, typed, alpha, statusA, 2 * tiles,
+                                                                   ticket);
                     SPH_CHECK_LAUNCH(c);
-                    bal_hash_kernel<<<blocks, 256, 0, c->stream>>>(n, p4, owner, ptype, ctl, A, B, T, hmax, bh);
+                    bal_hash_kernel<<<blocks, 256, 0, c->stream>>>(n, p4, owner, ptype, ctl, A, B, T, hmax, bh, code);
                     SPH_CHECK_LAUNCH(c);
                     bal_pair_select_kernel<<<1, kBalBins, 0, c->stream>>>(ctl, hmax);
                     SPH_CHECK_LAUNCH(c);
-                    bal_ties_kernel<<<div_up(n, 256), 256, 0, c->stream>>>(n, owner, ptype, bh, ctl, A, B, T, tieA, tieB);
-                    SPH_CHECK_LAUNCH(c);
-                    int rc = launch_scan_exclusive(c, n, tieA, rankA, nullptr);
-                    if (rc != SPH_OK) return rc;
-                    rc = launch_scan_exclusive(c, n, tieB, rankB, nullptr);
-                    if (rc != SPH_OK) return rc;
-                    bal_swap_kernel<<<div_up(n, 256), 256, 0, c->stream>>>(n, p4, owner, ptype, bh, ctl, A, B, T,
-                                                                          rankA, rankB);
+                    bal_swap_kernel<<<(unsigned)tiles, kBalThreads, 0, c->stream>>>(n, p4, owner, code, ctl, A, B, T,
+                                                                                  statusA, statusB, ticket);
                     SPH_CHECK_LAUNCH(c);
                 }
     }

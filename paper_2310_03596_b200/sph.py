@@ -385,15 +385,16 @@ class Context:
         self._chk(rc, "sph_step")
         return out
 
-    def sph_balance(self, posm: torch.Tensor, owner: torch.Tensor, hmax: int = 1000):
+    def sph_balance(self, posm: torch.Tensor, owner: torch.Tensor, hmax: int = 1000, want_hash: bool = True):
         """One balancing sweep over all owner pairs (NEXT-2): `owner` is updated in
-        place; returns (bal_hash [n] int32, swapped [1] int64)."""
+        place; returns (bal_hash [n] int32 or None, swapped [1] int64).  The hashes are an optional
+        product of the C call (bal_hash = NULL): want_hash=False skips their 4-byte scatter."""
         n = int(posm.shape[0])
-        bh = self._i32(max(n, 1))
+        bh = self._i32(max(n, 1)) if want_hash else None
         sw = torch.zeros(1, dtype=torch.int64, device=self.device)
         self._chk(self.lib.sph_balance(self.handle, n, posm.data_ptr(), owner.data_ptr(), int(hmax),
-                                       bh.data_ptr(), sw.data_ptr()), "sph_balance")
-        return bh[:n], sw
+                                       _ptr(bh), sw.data_ptr()), "sph_balance")
+        return (bh[:n] if want_hash else None), sw
 
     def sph_balance_types(self, posm: torch.Tensor, owner: torch.Tensor, ptype: torch.Tensor, n_types: int,
                           alpha: float = 0.1, hmax: int = 1000):

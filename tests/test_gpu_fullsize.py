@@ -152,3 +152,104 @@ def test_config3_full_size(sph, oracle):
     """configs[3], the irregular geometry as stated (22.0 M particles: plate + 8 cylinders, long
     runs of empty buckets, 16 owners by recursive coordinate bisection)."""
     _fullsize_case(sph, oracle, 3, steps_before=1, expect_boundary=(0.05, 0.35))
+
+
+# ------------------------------------------------------------------ NEXT items at full size
+def _balance_case(sph, oracle, w, sweeps):
+    """sph_balance against orc_balance, bit-exact: labels, hashes, swap count."""
+    g = w.n_owners
+    ctx = sph.Context.for_workload(w)
+    posm = torch.from_numpy(w.posm).cuda()
+    own_gpu = torch.from_numpy(w.owner.copy()).cuda()
+    own_ref = w.owner.copy()
+    total = 0
+    for sweep in range(sweeps):
+        bh, sw = ctx.sph_balance(posm, own_gpu)
+        torch.cuda.synchronize()
+        own_ref, k, bh_ref = oracle.balance(w.posm, own_ref, g)
+        assert int(sw.cpu()[0]) == k, (sweep, int(sw.cpu()[0]), k)
+        np.testing.assert_array_equal(bh.cpu().numpy(), bh_ref, err_msg=f"bal_hash sweep {sweep}")
+        np.testing.assert_array_equal(own_gpu.cpu().numpy(), own_ref, err_msg=f"owner sweep {sweep}")
+        total += k
+    np.testing.assert_array_equal(np.bincount(own_ref, minlength=g), np.bincount(w.owner, minlength=g))
+    ctx.close()
+    return total
+
+
+def test_balance_config2_full_size(sph, oracle):
+    """configs[2] (8 M particles, 16 owners, 120 pairs): two consecutive sweeps.  At this size the
+    grid-stride loops of the hash pass take several iterations, pass 2 spans 1 954 tiles and the
+    per-owner fixed-point sums exceed 2^40."""
+    assert _balance_case(sph, oracle, wl.config(2), sweeps=2) > 0
+
+
+@pytest.mark.skipif(os.environ.get("SPH_SKIP_64M") == "1", reason="SPH_SKIP_64M=1")
+def test_balance_config4_full_size(sph, oracle):
+    """configs[4] (64 M particles, random labels): one sweep, bit-exact (the workload of
+    bench.py's next2_balance block)."""
+    assert _balance_case(sph, oracle, wl.config(4), sweeps=1) > 0
+
+
+def test_balance_types_full_size(sph, oracle):
+    """sph_balance_types on 2.4 M particles, 5 owners, 3 types, alpha = 0.1."""
+    w = wl.lattice_block(200, 120, 100, 0.1, 41, owners=("random", 5))
+    nt = 3
+    ptype = np.random.default_rng(141).integers(0, nt, w.n).astype(np.int32)
+    ctx = sph.Context.for_workload(w)
+    posm = torch.from_numpy(w.posm).cuda()
+    pt = torch.from_numpy(ptype).cuda()
+    own_gpu = torch.from_numpy(w.owner.copy()).cuda()
+    bh, sw = ctx.sph_balance_types(posm, own_gpu, pt, nt, 0.1)
+    torch.cuda.synchronize()
+    own_ref, k, bh_ref = oracle.balance_types(w.posm, w.owner.copy(), ptype, 5, nt, alpha=0.1)
+    assert int(sw.cpu()[0]) == k and k > 0
+    np.testing.assert_array_equal(bh.cpu().numpy(), bh_ref)
+    np.testing.assert_array_equal(own_gpu.cpu().numpy(), own_ref)
+    for t in range(nt):
+        np.testing.assert_array_equal(np.bincount(own_ref[ptype == t], minlength=5),
+                                      np.bincount(w.owner[ptype == t], minlength=5))
+    ctx.close()
+
+
+def test_split_passes_config1_full_size(sph, oracle):
+    """sph_interact_split (steps e / f) on configs[1] (1 M particles, 4 slabs) after
+    3 steps: each pass on 3 000 sampled sorted positions against orc_interact_split (normalised by
+    the single pass's field maxima), pair counts add up, pass e + pass f = the single pass."""
+    w = wl.config(1)
+    ctx = sph.Context.for_workload(w)
+    state = sph.State.from_numpy(w.posm, w.velr, w.sig, w.owner)
+    for _ in range(3):
+        ctx.sph_step(state, w.dt)
+    hh = ctx.sph_hash(state.posm)
+    sh, perm = ctx.sph_sort(hh)
+    sst = ctx.sph_reorder(perm, state)
+    cs, ce = ctx.sph_cell_ranges(sh)
+    torch.cuda.synchronize()
+    p = parity.u32(perm).astype(np.int64)
+    posm, velr, sig, owner = (state.posm.cpu().numpy(), state.velr.cpu().numpy(), state.sig.cpu().numpy(),
+                              state.owner.cpu().numpy())
+    sp, sv, ss, so = posm[p], velr[p], np.ascontiguousarray(sig[:, p]), owner[p]
+    rng = np.random.default_rng(7)
+    # half of the sample from the slab interfaces (where pass f has work), half from anywhere
+    cross = np.nonzero(np.diff(so) != 0)[0]
+    idx = np.unique(np.concatenate([rng.integers(0, w.n, N_SAMPLE // 2),
+                                    rng.choice(cross, min(N_SAMPLE // 2, cross.size), replace=False)]))
+    args = (sp, sv, ss, parity.u32(sh), w.dims, parity.u32(cs), parity.u32(ce), w.h, w.K, w.G)
+    full = oracle.interact(*args, idx=idx)
+    scale = {k: max(np.abs(getattr(full, k)).max(), 1e-300) for k in ("drho", "acc", "dsig")}
+    g_all = ctx.sph_interact(sst, sh, cs, ce)
+    res = {}
+    for which in (1, 2):
+        drho, acc, dsig, pc = ctx.sph_interact_split(sst, sh, cs, ce, which)
+        torch.cuda.synchronize()
+        ref = oracle.interact_split(*args, so, which, idx=idx)
+        got = {"drho": drho.cpu().numpy(), "acc": acc.cpu().numpy()[:, :3], "dsig": dsig.cpu().numpy().T}
+        for name in ("drho", "acc", "dsig"):
+            err = np.abs(got[name][idx] - getattr(ref, name)).max() / scale[name]
+            assert err <= parity.RATE_TOL, (which, name, err)
+        res[which] = (got, int(pc.cpu()[0]))
+    assert res[2][1] > 0 and res[1][1] + res[2][1] == int(g_all[3].cpu()[0])
+    single = {"drho": g_all[0].cpu().numpy(), "acc": g_all[1].cpu().numpy()[:, :3], "dsig": g_all[2].cpu().numpy().T}
+    for name in ("drho", "acc", "dsig"):
+        assert np.abs(res[1][0][name] + res[2][0][name] - single[name]).max() <= parity.RATE_TOL * scale[name]
+    ctx.close()
