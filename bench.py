@@ -299,11 +299,13 @@ def run_ours(args, rank, world, local_rank):
         t_all, r_all = _t(lambda: ctx.sph_interact(st_, sh_, cs_, ce_))
         t_e, r_e = _t(lambda: ctx.sph_interact_split(st_, sh_, cs_, ce_, 1))
         t_f, r_f = _t(lambda: ctx.sph_interact_split(st_, sh_, cs_, ce_, 2))
+        t_ef, r_ef = _t(lambda: ctx.sph_interact_ef(st_, sh_, cs_, ce_))
         split = {"single_pass_ms": round(t_all, 4), "pass_e_ms": round(t_e, 4), "pass_f_ms": round(t_f, 4),
+                 "e_and_f_one_search_ms": round(t_ef, 4), "e_and_f_over_single": round(t_ef / t_all, 3),
                  "pairs_single": int(r_all[3].cpu()[0]), "pairs_e": int(r_e[3].cpu()[0]),
                  "pairs_f": int(r_f[3].cpu()[0]),
                  "note": "stand-alone sph_interact calls (pack pass and output allocation included)"}
-        del hh, sh_, pm_, st_, cs_, ce_, r_all, r_e, r_f
+        del hh, sh_, pm_, st_, cs_, ce_, r_all, r_e, r_f, r_ef
 
     # ---- NEXT-2 (not part of the step metric): one balancing sweep and what it does to the exchange set ----
     bal = None

@@ -209,6 +209,20 @@ int sph_balance_types(sph_ctx *ctx, int64_t n, const float *posm, int32_t *owner
                       int32_t n_types, double alpha, int32_t hmax, int32_t *bal_hash,
                       unsigned long long *swapped);
 
+/* NEXT-3, both passes from ONE neighbour search: the stencil is searched once per particle, the
+ * accepted neighbours are split by owner label, and the sums of step e (same label)
+ * and of step f (other labels) are accumulated one after the other into two sets of
+ * rate arrays.  Equal to sph_interact_split(which = 1) and (which = 2) up to rounding, at the cost
+ * of one search instead of two.  (On one GPU the two steps have no exchange between them to wait
+ * for; a multi-GPU run that overlaps step e with the broadcast would call the split passes.)
+ * sorted_h: per-particle smoothing lengths in sorted order as in sph_interact_varh, or NULL for the
+ * uniform sph_params.h.  pair_counts dev [2] out: accepted ordered pairs of step e and of step f
+ * (zeroed by the call).  All arrays dev, indexed by sorted position, as in sph_interact. */
+int sph_interact_ef(sph_ctx *ctx, int64_t n, const sph_state *sorted, const float *sorted_h,
+                    const uint32_t *sorted_hash, const uint32_t *cell_start, const uint32_t *cell_end,
+                    float *drho_e, float *acc_e, float *const dsig_e[6], float *drho_f, float *acc_f,
+                    float *const dsig_f[6], unsigned long long *pair_counts);
+
 /* NEXT-4, second half -- per-particle smoothing lengths ("cubic
  * buckets of size 2h with h the maximum smoothing length of the particles"; PAPER.md:54 particle
  * types "with different smoothing lengths").  Readings H1-H3: the bucket grid

@@ -8,7 +8,8 @@ namespace sphb {
 int launch_interact(sph_ctx *c, int64_t n, const sph_state *sorted, const uint32_t *sorted_hash,
                     const uint32_t *cs, const uint32_t *ce, float *drho, float *acc,
                     float *const dsig[6], unsigned long long *pair_count, const sph_state *fuse_out,
-                    const uint32_t *perm, float dt, int mode, const float *sorted_h)
+                    const uint32_t *perm, float dt, int mode, const float *sorted_h, float *drho_f, float *acc_f,
+                    float *const dsig_f[6])
 {
     if (n == 0) return SPH_OK;
     InteractIn in;
@@ -29,6 +30,19 @@ int launch_interact(sph_ctx *c, int64_t n, const sph_state *sorted, const uint32
         out.o_posm = reinterpret_cast<float4 *>(fuse_out->posm);
         out.o_velr = reinterpret_cast<float4 *>(fuse_out->velr);
         for (int i = 0; i < 6; ++i) out.o_sig[i] = fuse_out->sig[i];
+    }
+    if (mode == kPassBoth) {
+        // steps e and f from one neighbour search: a second set of rate arrays (step f)
+        InteractOut of = out;
+        of.drho = drho_f;
+        of.acc = reinterpret_cast<float4 *>(acc_f);
+        for (int i = 0; i < 6; ++i) of.dsig[i] = dsig_f[i];
+        if (c->params.flags & SPH_FLAG_INTERACT_DIRECT) {
+            int rc = launch_interact_direct(c, n, in, sorted_hash, cs, ce, out, pair_count, kPassLocal);
+            if (rc != SPH_OK) return rc;
+            return launch_interact_direct(c, n, in, sorted_hash, cs, ce, of, pair_count + 1, kPassRemote);
+        }
+        return launch_interact_tiled(c, n, in, sorted_hash, cs, ce, out, pair_count, mode, &of);
     }
     if (c->params.flags & SPH_FLAG_INTERACT_DIRECT)
         return launch_interact_direct(c, n, in, sorted_hash, cs, ce, out, pair_count, mode);

@@ -21,6 +21,8 @@ struct InteractIn {
 // Which neighbours a pass takes: 0 = all (steps e and f as one loop),
 // 1 = step e alone (same owner label), 2 = step f alone (other owner labels).
 constexpr int kPassAll = 0, kPassLocal = 1, kPassRemote = 2;
+// 3 = both split passes from ONE neighbour search (two rate sets; sph_interact_ef)
+constexpr int kPassBoth = 3;
 struct InteractOut {
     float *drho;          // rates, indexed by sorted position; all three NULL = not wanted
     float4 *acc;
@@ -351,6 +353,6 @@ int launch_interact_direct(sph_ctx *c, int64_t n, const InteractIn &in, const ui
                            unsigned long long *pair_count, int mode);
 int launch_interact_tiled(sph_ctx *c, int64_t n, const InteractIn &in, const uint32_t *sorted_hash,
                           const uint32_t *cs, const uint32_t *ce, const InteractOut &out,
-                          unsigned long long *pair_count, int mode);
+                          unsigned long long *pair_count, int mode, const InteractOut *out_f = nullptr);
 
 }  // namespace sphb

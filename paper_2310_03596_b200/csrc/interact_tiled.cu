@@ -183,8 +183,9 @@ template <bool kCount, int kMode, bool kVarH>
 __global__ void __launch_bounds__(kTW * 32, 2)
 interact_tiled_kernel(Packed rec, InteractIn in, const uint32_t *__restrict__ cs,
                       const uint32_t *__restrict__ ce, Grid g, Consts k, InteractOut out,
-                      unsigned long long *pair_count, int tiles_x, int tiles_y)
+                      unsigned long long *pair_count, int tiles_x, int tiles_y, InteractOut out_f)
 {
+    // kMode == kPassBoth: step e goes to `out`, step f to `out_f`; pair_count[0] / [1] likewise
     extern __shared__ __align__(16) unsigned char smem_raw[];
     TileSmem &sm = *reinterpret_cast<TileSmem *>(smem_raw);
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
@@ -236,11 +237,17 @@ interact_tiled_kernel(Packed rec, InteractIn in, const uint32_t *__restrict__ cs
         asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
         asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
     }
-    uint32_t my_pairs = 0, my_self = 0;
+    uint32_t my_pairs = 0, my_self = 0, my_pairs_f = 0;
     if (total > kCap) {
         // window too large for shared memory (very dense region): direct walk, warp = bucket
-        for (int i = lane; i < nt; i += 32)
-            my_pairs += direct_particle((int64_t)tb0 + i, cxb, cyb, cz, in, cs, ce, g, k, out, kMode);
+        for (int i = lane; i < nt; i += 32) {
+            if (kMode == kPassBoth) {
+                my_pairs += direct_particle((int64_t)tb0 + i, cxb, cyb, cz, in, cs, ce, g, k, out, kPassLocal);
+                my_pairs_f += direct_particle((int64_t)tb0 + i, cxb, cyb, cz, in, cs, ce, g, k, out_f, kPassRemote);
+            } else {
+                my_pairs += direct_particle((int64_t)tb0 + i, cxb, cyb, cz, in, cs, ce, g, k, out, kMode);
+            }
+        }
     } else {
         __syncthreads();  // mbarrier initialised before the copies are issued against it
         if (warp == 0) {
@@ -337,8 +344,14 @@ interact_tiled_kernel(Packed rec, InteractIn in, const uint32_t *__restrict__ cs
 
         // a bucket whose table overflowed is walked directly by its own warp
         if (nt > 0 && sm.cand_len[warp] < 0)
-            for (int i = lane; i < nt; i += 32)
-                my_pairs += direct_particle((int64_t)tb0 + i, cxb, cyb, cz, in, cs, ce, g, k, out, kMode);
+            for (int i = lane; i < nt; i += 32) {
+                if (kMode == kPassBoth) {
+                    my_pairs += direct_particle((int64_t)tb0 + i, cxb, cyb, cz, in, cs, ce, g, k, out, kPassLocal);
+                    my_pairs_f += direct_particle((int64_t)tb0 + i, cxb, cyb, cz, in, cs, ce, g, k, out_f, kPassRemote);
+                } else {
+                    my_pairs += direct_particle((int64_t)tb0 + i, cxb, cyb, cz, in, cs, ce, g, k, out, kMode);
+                }
+            }
 
         // ---- work units: lane b < kNB keeps the record of bucket b -----------------------------
         int l_nt = 0, l_tsm = 0, l_wp = 0, l_ng = 0;
@@ -405,17 +418,23 @@ interact_tiled_kernel(Packed rec, InteractIn in, const uint32_t *__restrict__ cs
             }
             // keeps, of the 4 fresh mask bits of one candidate, those the pass takes:
             // same-owner pairs (step e) or other-owner pairs (step f)
-            auto owner_filter = [&](uint32_t &mask, uint32_t e) {
+            // (kPassBoth keeps every accepted pair and records the equality nibble in a second word)
+            auto owner_filter = [&](uint32_t &mask, uint32_t &eqw, uint32_t e) {
                 if (kMode == kPassAll) return;
                 const uint32_t oj = sm.own[e >> 4];
-                uint32_t eq = 0;
-#pragma unroll
-                for (int dd = 0; dd < 4; ++dd) eq |= (((own4 >> (8 * dd)) & 0xFFu) == oj ? 1u : 0u) << dd;
-                mask &= ~0xFu | (kMode == kPassLocal ? eq : ~eq);
+                // four byte compares at once: (own4 ^ oj oj oj oj) has a zero byte where the labels
+                // agree (labels < 32, absent targets 0xFF never match); exact per-byte zero test
+                // (no carry crosses a byte), then the four flags are gathered into a nibble
+                const uint32_t x = own4 ^ (oj * 0x01010101u);
+                const uint32_t nz = ((x & 0x7F7F7F7Fu) + 0x7F7F7F7Fu) | x;     // bit 7 of a byte set <=> byte != 0
+                const uint32_t eq = (((~nz & 0x80808080u) >> 7) * 0x01020408u) >> 24;   // byte d -> bit d
+                if (kMode == kPassBoth) eqw = (eqw << 4) | eq;
+                else mask &= ~0xFu | (kMode == kPassLocal ? eq : ~eq);
             };
 
             // ---- phase 1: the whole table, bit 4 s + d of mask word s / 8 <- chunk s, slot d ----
             uint32_t m0 = 0, m1 = 0, m2 = 0;
+            uint32_t q0 = 0, q1 = 0, q2 = 0;   // kPassBoth: same-owner bits, aligned with m0..m2
             const int nch = Wp >> 5;
             const uint16_t *cb = cand + lane;
 #pragma unroll 1
@@ -424,7 +443,7 @@ interact_tiled_kernel(Packed rec, InteractIn in, const uint32_t *__restrict__ cs
                 const float4 pa = ld_rec(sm.A, ce_);
                 test_push2(m2, pa, ax23, ay23, az23, nt23);
                 test_push2(m2, pa, ax01, ay01, az01, nt01);
-                owner_filter(m2, ce_);
+                owner_filter(m2, q2, ce_);
             }
 #pragma unroll 4
             for (int s = min(nch, 16) - 1; s >= 8; --s) {
@@ -432,7 +451,7 @@ interact_tiled_kernel(Packed rec, InteractIn in, const uint32_t *__restrict__ cs
                 const float4 pa = ld_rec(sm.A, ce_);
                 test_push2(m1, pa, ax23, ay23, az23, nt23);
                 test_push2(m1, pa, ax01, ay01, az01, nt01);
-                owner_filter(m1, ce_);
+                owner_filter(m1, q1, ce_);
             }
 #pragma unroll 4
             for (int s = min(nch, 8) - 1; s >= 0; --s) {
@@ -440,7 +459,7 @@ interact_tiled_kernel(Packed rec, InteractIn in, const uint32_t *__restrict__ cs
                 const float4 pa = ld_rec(sm.A, ce_);
                 test_push2(m0, pa, ax23, ay23, az23, nt23);
                 test_push2(m0, pa, ax01, ay01, az01, nt01);
-                owner_filter(m0, ce_);
+                owner_filter(m0, q0, ce_);
             }
             // every quarter collects the bits of its own target: slot d of the lanes of quarter
             // q ^ d.  Afterwards bit beta of word w <-> table position 256 w + t + 8 (beta ^ q).
@@ -455,19 +474,29 @@ interact_tiled_kernel(Packed rec, InteractIn in, const uint32_t *__restrict__ cs
                     const uint32_t c3 = __shfl_xor_sync(0xffffffffu, m2, 24);
                     m2 = (m2 & 0x11111111u) | (c1 & 0x22222222u) | (c2 & 0x44444444u) | (c3 & 0x88888888u);
                 }
+                if (kMode == kPassBoth) {
+                    auto xch = [&](uint32_t v) {
+                        const uint32_t v1 = __shfl_xor_sync(0xffffffffu, v, 8), v2 = __shfl_xor_sync(0xffffffffu, v, 16);
+                        const uint32_t v3 = __shfl_xor_sync(0xffffffffu, v, 24);
+                        return (v & 0x11111111u) | (v1 & 0x22222222u) | (v2 & 0x44444444u) | (v3 & 0x88888888u);
+                    };
+                    q0 = xch(q0); q1 = xch(q1); q2 = xch(q2);
+                }
             }
             // ---- phase 2: lane t of quarter q owns the accepted candidates of target q whose record
             //      index is = t (mod 8) and evaluates them straight from its mask words, two per
             //      round.  The 8 gathers of a quarter-warp always fall into 8 distinct 16-byte bank
             //      groups (conflict-free by construction); a lane that has run out of bits gathers
             //      the dummy record of its own class, which contributes exactly zero. -------------
-            const int c = __popc(m0) + __popc(m1) + __popc(m2);
-            const int rounds = (int)__reduce_max_sync(0xffffffffu, (unsigned)((c + 1) >> 1));
             float4 tv = make_float4(0.f, 0.f, 0.f, 0.f);
             float th = 1.0f;   // the target's own smoothing length (NEXT-4)
             if (my_valid) tv = sm.B[tbase + my_t];
             if (kVarH && my_valid) th = sm.C[tbase + my_t].z;
             const f32x2 tpxy = pk(tp.x, tp.y), tvxy = pk(tv.x, tv.y);
+            // phase 2 + reduction + parking of one set of mask words (kPassBoth runs it twice)
+            auto pass2 = [&](uint32_t u0, uint32_t u1, uint32_t u2, int slot, uint32_t &cnt) {
+            const int c = __popc(u0) + __popc(u1) + __popc(u2);
+            const int rounds = (int)__reduce_max_sync(0xffffffffu, (unsigned)((c + 1) >> 1));
             PairAccum2 S;
             S.clear();
             {
@@ -475,7 +504,7 @@ interact_tiled_kernel(Packed rec, InteractIn in, const uint32_t *__restrict__ cs
                 // branch-free: refill the head word when it has run dry, take its highest bit
                 const uint32_t dummy = (uint32_t)(kDummy + t) * 16u;
                 const uint32_t cbase = smem_u32(cand + t);
-                uint32_t w = m0, w1 = m1, w2 = m2;
+                uint32_t w = u0, w1 = u1, w2 = u2;
                 uint32_t c0 = cbase, c1 = cbase + 512u, c2 = cbase + 1024u;
                 if (w1 == 0u) { w1 = w2; c1 = c2; w2 = 0u; }
                 if (w == 0u) { w = w1; c0 = c1; w1 = w2; c1 = c2; w2 = 0u; }
@@ -503,7 +532,7 @@ interact_tiled_kernel(Packed rec, InteractIn in, const uint32_t *__restrict__ cs
                     const float r2 = S.template add<kVarH>(tpxy, tp.z, tvxy, tv.z, pa, pb, pc, pd, -k.half_inv_h, th);
                     // exact test (phase 1 has a rounding margin; with per-particle lengths it runs on 2 h_max)
                     const float hs = th + pc.z;
-                    if (kCount && r2 < (kVarH ? hs * hs : k.support2)) ++my_pairs;
+                    if (kCount && r2 < (kVarH ? hs * hs : k.support2)) ++cnt;
                 };
 #pragma unroll 1
                 for (int r = 0; r < rounds; ++r) {
@@ -518,7 +547,7 @@ interact_tiled_kernel(Packed rec, InteractIn in, const uint32_t *__restrict__ cs
                 float v[16];
                 S.unpack(v);
                 reduce8_transposed(v, t);
-                float *row = acc[parked * 4 + q];
+                float *row = acc[slot * 4 + q];
                 const int idx = ((t & 4) << 1) + ((t & 2) << 1) + ((t & 1) << 1);
                 row[idx] = v[0];
                 row[idx + 1] = v[1];
@@ -527,8 +556,16 @@ interact_tiled_kernel(Packed rec, InteractIn in, const uint32_t *__restrict__ cs
                     row[17] = __int_as_float(tbase + my_t);
                 }
             }
+            };
+            if (kMode == kPassBoth) {
+                // step e: same-owner pairs -> slot 0 -> out; step f: the others -> slot 1 -> out_f
+                pass2(m0 & q0, m1 & q1, m2 & q2, 0, my_pairs);
+                pass2(m0 & ~q0, m1 & ~q1, m2 & ~q2, 1, my_pairs_f);
+            } else {
+                pass2(m0, m1, m2, parked, my_pairs);
+            }
             if (kMode != kPassRemote && my_valid && t == 0) ++my_self;  // the self pair is not a pair (reading S15)
-            ++parked;
+            parked = kMode == kPassBoth ? 2 : parked + 1;   // kPassBoth parked two sets of this unit
             if (parked == kSlots / 4 || gi + kTW >= NG) {
                 // ---- epilogue: one lane per parked target (O8, stores) ------------------------
                 __syncwarp();
@@ -554,7 +591,8 @@ interact_tiled_kernel(Packed rec, InteractIn in, const uint32_t *__restrict__ cs
                         si[3] = rc.y * rho2; si[4] = rd.x * rho2; si[5] = rd.y * rho2;
                         float4 pos_i = make_float4(0.f, 0.f, 0.f, 0.f);
                         if (out.perm) pos_i = __ldg(in.posm + i);
-                        finish_particle(Rr, si, rho, k, out, (int64_t)i, pos_i, rb.x, rb.y, rb.z);
+                        const InteractOut &oo = (kMode == kPassBoth && lane >= 4) ? out_f : out;
+                        finish_particle(Rr, si, rho, k, oo, (int64_t)i, pos_i, rb.x, rb.y, rb.z);
                     }
                 }
                 __syncwarp();
@@ -592,12 +630,16 @@ interact_tiled_kernel(Packed rec, InteractIn in, const uint32_t *__restrict__ cs
     if (kCount) {
         const uint32_t tot = __reduce_add_sync(0xffffffffu, my_pairs) - __reduce_add_sync(0xffffffffu, my_self);
         if (lane == 0 && tot) atomicAdd(pair_count, (unsigned long long)tot);
+        if (kMode == kPassBoth) {
+            const uint32_t tf = __reduce_add_sync(0xffffffffu, my_pairs_f);
+            if (lane == 0 && tf) atomicAdd(pair_count + 1, (unsigned long long)tf);
+        }
     }
 }
 
 int launch_interact_tiled(sph_ctx *c, int64_t n, const InteractIn &in, const uint32_t *sorted_hash,
                           const uint32_t *cs, const uint32_t *ce, const InteractOut &out,
-                          unsigned long long *pair_count, int mode)
+                          unsigned long long *pair_count, int mode, const InteractOut *out_f)
 {
     (void)sorted_hash;
     Packed rec;
@@ -617,7 +659,8 @@ int launch_interact_tiled(sph_ctx *c, int64_t n, const InteractIn &in, const uin
             (const void *)interact_tiled_kernel<true, kPassAll, false>, (const void *)interact_tiled_kernel<false, kPassAll, false>,
             (const void *)interact_tiled_kernel<true, kPassLocal, false>, (const void *)interact_tiled_kernel<true, kPassRemote, false>,
             (const void *)interact_tiled_kernel<true, kPassAll, true>, (const void *)interact_tiled_kernel<false, kPassAll, true>,
-            (const void *)interact_tiled_kernel<true, kPassLocal, true>, (const void *)interact_tiled_kernel<true, kPassRemote, true>};
+            (const void *)interact_tiled_kernel<true, kPassLocal, true>, (const void *)interact_tiled_kernel<true, kPassRemote, true>,
+            (const void *)interact_tiled_kernel<true, kPassBoth, false>, (const void *)interact_tiled_kernel<true, kPassBoth, true>};
         for (const void *f : fns) SPH_CUDA_TRY(c, cudaFuncSetAttribute(f, cudaFuncAttributeMaxDynamicSharedMemorySize, smem));
         c->attr_interact = true;
     }
@@ -632,12 +675,15 @@ int launch_interact_tiled(sph_ctx *c, int64_t n, const InteractIn &in, const uin
     unsigned long long *pc = (mode == kPassAll || pair_count) ? pair_count : c->s_pair_count;
 #define SPH_LAUNCH_TILED(CNT, MODE, VH)                                                        \
     interact_tiled_kernel<CNT, MODE, VH><<<gr, kTW * 32, smem, c->stream>>>(                     \
-        rec, in, cs, ce, c->grid, kc, out, pc, tiles_x, tiles_y)
+        rec, in, cs, ce, c->grid, kc, out, pc, tiles_x, tiles_y, out_f ? *out_f : out)
     if (mode == kPassAll) {
         if (pair_count) { if (vh) SPH_LAUNCH_TILED(true, kPassAll, true); else SPH_LAUNCH_TILED(true, kPassAll, false); }
         else            { if (vh) SPH_LAUNCH_TILED(false, kPassAll, true); else SPH_LAUNCH_TILED(false, kPassAll, false); }
     } else if (mode == kPassLocal) {
         if (vh) SPH_LAUNCH_TILED(true, kPassLocal, true); else SPH_LAUNCH_TILED(true, kPassLocal, false);
+    } else if (mode == kPassBoth) {
+        if (!out_f || !pair_count) return SPH_EINVAL;   // two rate sets, pair_count[2]
+        if (vh) SPH_LAUNCH_TILED(true, kPassBoth, true); else SPH_LAUNCH_TILED(true, kPassBoth, false);
     } else {
         if (vh) SPH_LAUNCH_TILED(true, kPassRemote, true); else SPH_LAUNCH_TILED(true, kPassRemote, false);
     }

@@ -270,6 +270,21 @@ int sph_interact_split(sph_ctx *c, int64_t n, const sph_state *sorted, const uin
                            which);
 }
 
+int sph_interact_ef(sph_ctx *c, int64_t n, const sph_state *sorted, const float *sorted_h,
+                    const uint32_t *sorted_hash, const uint32_t *cs, const uint32_t *ce, float *drho_e,
+                    float *acc_e, float *const dsig_e[6], float *drho_f, float *acc_f, float *const dsig_f[6],
+                    unsigned long long *pair_counts)
+{
+    if (!n_ok(c, n) || !state_ok(sorted) || !sorted_hash || !cs || !ce || !drho_e || !acc_e || !dsig_e || !drho_f ||
+        !acc_f || !dsig_f || !pair_counts)
+        return SPH_EINVAL;
+    for (int i = 0; i < 6; ++i)
+        if (!dsig_e[i] || !dsig_f[i]) return SPH_EINVAL;
+    SPH_CUDA_TRY(c, cudaMemsetAsync(pair_counts, 0, 2 * sizeof(unsigned long long), c->stream));
+    return launch_interact(c, n, sorted, sorted_hash, cs, ce, drho_e, acc_e, dsig_e, pair_counts, nullptr, nullptr,
+                           0.f, 3, sorted_h, drho_f, acc_f, dsig_f);
+}
+
 int sph_integrate(sph_ctx *c, int64_t n, float dt, const sph_state *in, const float *drho,
                   const float *acc, const float *const dsig[6], const sph_state *out)
 {

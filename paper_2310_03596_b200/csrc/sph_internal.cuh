@@ -130,7 +130,8 @@ int launch_interact(sph_ctx *c, int64_t n, const sph_state *sorted, const uint32
                     float *const dsig[6], unsigned long long *pair_count,
                     const sph_state *fuse_out /* NULL = rates only */, const uint32_t *perm, float dt,
                     int mode = 0 /* 0 all, 1 same-owner, 2 other-owner neighbours */,
-                    const float *sorted_h = nullptr /* NEXT-4: per-particle smoothing lengths */);
+                    const float *sorted_h = nullptr /* NEXT-4: per-particle smoothing lengths */,
+                    float *drho_f = nullptr, float *acc_f = nullptr, float *const dsig_f[6] = nullptr /* mode 3 */);
 int launch_integrate(sph_ctx *c, int64_t n, float dt, const sph_state *in, const float *drho,
                      const float *acc, const float *const dsig[6], const sph_state *out,
                      const uint32_t *scatter_perm /* NULL = elementwise */);

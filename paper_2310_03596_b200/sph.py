@@ -30,7 +30,7 @@ TIMING_SLOTS = 32          # steps held by the library's ring of stage events (s
 EXPORTS = (
     "sph_create", "sph_destroy", "sph_hash", "sph_sort", "sph_reorder", "sph_cell_ranges",
     "sph_comm_hash", "sph_interact", "sph_integrate", "sph_step", "sph_step_host", "sph_pack_boundary",
-    "sph_interact_split", "sph_interact_varh", "sph_step_varh", "sph_balance", "sph_balance_types", "sph_enable_timing", "sph_get_timing", "sph_launch_count", "sph_strerror",
+    "sph_interact_split", "sph_interact_varh", "sph_step_varh", "sph_interact_ef", "sph_balance", "sph_balance_types", "sph_enable_timing", "sph_get_timing", "sph_launch_count", "sph_strerror",
     "sph_last_cuda_error",
 )
 
@@ -74,6 +74,8 @@ def load_library() -> C.CDLL:
     lib.sph_interact_split.argtypes = [vp, i64, sp, vp, vp, vp, i32, vp, vp, C.POINTER(vp * 6), vp]
     lib.sph_interact_varh.argtypes = [vp, i64, sp, vp, vp, vp, vp, i32, vp, vp, C.POINTER(vp * 6), vp]
     lib.sph_step_varh.argtypes = [vp, i64, f32, sp, vp] + [vp] * 11 + [C.POINTER(vp * 6), vp]
+    lib.sph_interact_ef.argtypes = [vp, i64, sp, vp, vp, vp, vp, vp, vp, C.POINTER(vp * 6), vp, vp,
+                                    C.POINTER(vp * 6), vp]
     lib.sph_integrate.argtypes = [vp, i64, f32, sp, vp, vp, C.POINTER(vp * 6), sp]
     lib.sph_step.argtypes = [vp, i64, f32, sp] + [vp] * 11 + [C.POINTER(vp * 6), vp]
     lib.sph_step_host.argtypes = [vp, i64, f32, i32, sp, vp, vp, vp]
@@ -331,6 +333,21 @@ class Context:
                   "sph_interact_varh")
         return drho, acc, dsig, pc
 
+    def sph_interact_ef(self, sorted_state: State, sorted_hash, cell_start, cell_end, sorted_h=None):
+        """Steps e and f from one neighbour search: returns ((drho, acc, dsig) of
+        step e, (drho, acc, dsig) of step f, pair_counts [2] int64)."""
+        n = sorted_state.n
+        e = (self._f32(n), self._f32(n, 4), self._f32(6, n))
+        f = (self._f32(n), self._f32(n, 4), self._f32(6, n))
+        pc = torch.zeros(2, dtype=torch.int64, device=self.device)
+        s = sorted_state._c()
+        de, df = _six(e[2]), _six(f[2])
+        self._chk(self.lib.sph_interact_ef(self.handle, n, C.byref(s), _ptr(sorted_h), sorted_hash.data_ptr(),
+                                           cell_start.data_ptr(), cell_end.data_ptr(), e[0].data_ptr(),
+                                           e[1].data_ptr(), C.byref(de), f[0].data_ptr(), f[1].data_ptr(),
+                                           C.byref(df), pc.data_ptr()), "sph_interact_ef")
+        return e, f, pc
+
     def sph_step_varh(self, state: State, h: torch.Tensor, dt, out: StepOutputs | None = None,
                       pair_count: torch.Tensor | None = None):
         """sph_step with a smoothing length per particle (h [n] f32 in id order, NEXT-4)."""
@@ -442,6 +459,7 @@ def sph_comm_hash(ctx, *a, **k): return ctx.sph_comm_hash(*a, **k)
 def sph_interact(ctx, *a, **k): return ctx.sph_interact(*a, **k)
 def sph_interact_split(ctx, *a, **k): return ctx.sph_interact_split(*a, **k)
 def sph_interact_varh(ctx, *a, **k): return ctx.sph_interact_varh(*a, **k)
+def sph_interact_ef(ctx, *a, **k): return ctx.sph_interact_ef(*a, **k)
 def sph_step_varh(ctx, *a, **k): return ctx.sph_step_varh(*a, **k)
 def sph_integrate(ctx, *a, **k): return ctx.sph_integrate(*a, **k)
 def sph_step(ctx, *a, **k): return ctx.sph_step(*a, **k)

@@ -412,6 +412,53 @@ def test_balance_types_matches_oracle_bit_exact(sph, oracle, g, nt, alpha):
     ctx.close()
 
 
+@pytest.mark.parametrize("flags", [0, 1], ids=["tiled", "direct"])
+@pytest.mark.parametrize("make,dense", [(lambda: wl.t1b(side=18, seed=1105), False), (lambda: wl.config(2, side=33), False),
+                                        (lambda: wl.config(4, side=29), True)], ids=["t1b", "cfg2", "cfg4-dense"])
+def test_interact_ef_one_search_two_rate_sets(sph, oracle, make, dense, flags):
+    """sph_interact_ef: steps e and f from ONE neighbour search.  Each rate set
+    against orc_interact_split, pair counts exact against the split calls, e + f = single pass.
+    The dense case (lattice squeezed to 0.85) drives tiles into the direct-walk fallbacks."""
+    w = make()
+    if w.sig.max() == 0:
+        rng = np.random.default_rng(78)
+        w.sig[:] = (rng.standard_normal((6, w.n)) * 1e-3).astype(np.float32)
+        w.velr[:, 3] = (1.0 + (rng.random(w.n) * 2 - 1) * 0.01).astype(np.float32)
+    if dense:
+        w.posm[:, :3] *= np.float32(0.85)
+    ctx = sph.Context.for_workload(w, flags=flags)
+    st = sph.State.from_numpy(w.posm, w.velr, w.sig, w.owner)
+    sh, perm = ctx.sph_sort(ctx.sph_hash(st.posm))
+    sst = ctx.sph_reorder(perm, st)
+    cs, ce = ctx.sph_cell_ranges(sh)
+    e, f, pc = ctx.sph_interact_ef(sst, sh, cs, ce)
+    single = ctx.sph_interact(sst, sh, cs, ce)
+    se = ctx.sph_interact_split(sst, sh, cs, ce, 1)
+    sf = ctx.sph_interact_split(sst, sh, cs, ce, 2)
+    torch.cuda.synchronize()
+    p = parity.u32(perm).astype(np.int64)
+    args = (w.posm[p], w.velr[p], np.ascontiguousarray(w.sig[:, p]), parity.u32(sh), w.dims, parity.u32(cs),
+            parity.u32(ce), w.h, w.K, w.G)
+    full = oracle.interact(*args)
+    scale = {k: max(np.abs(getattr(full, k)).max(), 1e-300) for k in ("drho", "acc", "dsig")}
+    pcs = pc.cpu().numpy()
+    assert pcs[0] == int(se[3].cpu()[0]) and pcs[1] == int(sf[3].cpu()[0])
+    assert pcs[0] + pcs[1] == int(single[3].cpu()[0])
+    tot = {}
+    for which, got in ((1, e), (2, f)):
+        ref = oracle.interact_split(*args, w.owner[p], which)
+        g = {"drho": got[0].cpu().numpy(), "acc": got[1].cpu().numpy()[:, :3], "dsig": got[2].cpu().numpy().T}
+        for name in ("drho", "acc", "dsig"):
+            err = np.abs(g[name] - getattr(ref, name)).max() / scale[name]
+            assert err <= parity.RATE_TOL, (which, name, err)
+            tot[name] = tot.get(name, 0) + g[name]
+        assert abs(int(pcs[which - 1]) - ref.pair_count) <= max(1e-6 * ref.pair_count, 2)
+    sg = {"drho": single[0].cpu().numpy(), "acc": single[1].cpu().numpy()[:, :3], "dsig": single[2].cpu().numpy().T}
+    for name in ("drho", "acc", "dsig"):
+        assert np.abs(tot[name] - sg[name]).max() <= parity.RATE_TOL * scale[name], name
+    ctx.close()
+
+
 # ------------------------------------------------------------------ NEXT-4: per-particle smoothing lengths
 @pytest.mark.parametrize("flags", [0, 1], ids=["tiled", "direct"])
 @pytest.mark.parametrize("kind", [("species", 2, 0.75), ("random", 0.5), ("uniform",)],
