@@ -16,7 +16,7 @@
  *  - sph_ctx owns only scratch (radix-sort ping-pong buffers, histograms, tile status words,
  *    per-bucket owner masks, scan space, the sorted copy of the state used by sph_step).  It is
  *    sized for max_n particles and the grid of the sph_params given at creation.
- *  - Every entry point except sph_create / sph_destroy / sph_step_host only ENQUEUES work on the
+ *  - Every entry point except sph_create / sph_destroy / sph_step_host / sph_balance[_types] only ENQUEUES work on the
  *    ctx's stream and returns; outputs are valid once the caller synchronises that stream.
  *    No allocation and no host synchronisation happens on the hot path.  One ctx per host thread.
  *  - Return value: 0 = SPH_OK, negative = error (below).  No exception crosses this boundary.
@@ -191,6 +191,8 @@ int sph_pack_boundary(sph_ctx *ctx, int64_t n, int64_t m, const sph_state *state
  * ascending) swap labels.  Every owner keeps its particle count.  Exact arithmetic contract (so
  * that the labels have one correct value): Cg from 2^-16 fixed-point int64 coordinate sums, s in
  * fp64 without contraction.
+ * Unlike the stage calls this one SYNCHRONISES the ctx's stream once (the ids are first grouped by
+ * owner, and the sizes of the groups, read back once per sweep, size the launches of the pairs).
  * In: posm dev [n][4] in id order; hmax in 1 .. 1023 (the paper's typical value: 1000).
  * In/out: owner dev [n].  Out (optional, may be NULL): bal_hash dev [n] = the hash each particle
  * got in the last pair that involved it (0 if none); swapped dev scalar = particle pairs swapped. */

@@ -294,14 +294,7 @@ onesweep_kernel(int64_t n, const uint32_t *__restrict__ keys_in, const uint32_t 
     }
 }
 
-__global__ void __launch_bounds__(256) iota_copy_kernel(int64_t n, const uint32_t *__restrict__ hash,
-                                                        uint32_t *__restrict__ sorted_hash,
-                                                        uint32_t *__restrict__ perm)
-{
-    int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
-    if (i < n) { sorted_hash[i] = hash[i]; perm[i] = (uint32_t)i; }
-}
-
+// (moved up: used by the sort and by the partition)
 // the opt-in to > 48 KB of dynamic shared memory is per device: once per ctx (a ctx is bound to
 // the device that was current at sph_create)
 static int sort_smem_opt_in(sph_ctx *c)
@@ -313,6 +306,14 @@ static int sort_smem_opt_in(sph_ctx *c)
                                          (int)sizeof(SortSmem)));
     c->attr_sort = true;
     return SPH_OK;
+}
+
+__global__ void __launch_bounds__(256) iota_copy_kernel(int64_t n, const uint32_t *__restrict__ hash,
+                                                        uint32_t *__restrict__ sorted_hash,
+                                                        uint32_t *__restrict__ perm)
+{
+    int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (i < n) { sorted_hash[i] = hash[i]; perm[i] = (uint32_t)i; }
 }
 
 int launch_sort(sph_ctx *c, int64_t n, const uint32_t *hash, uint32_t *sorted_hash, uint32_t *perm)
@@ -387,40 +388,51 @@ __global__ void segment_offsets_kernel(const uint32_t *__restrict__ hist_excl, i
     if (g == n_labels) offsets[g] = m;
 }
 
-int launch_partition_by_label(sph_ctx *c, int64_t m, const uint32_t *ids, const int32_t *label, int n_labels,
-                              uint32_t *offsets, uint32_t *dest)
+// Stable partition of the implicit indices 0..m-1 by the keys in c->alt_keys (< 256): offsets
+// [n_labels + 1] = segment starts, *order = the indices in partition order (ctx scratch), dest
+// (optional) = destination of every index (the inverse map).
+int launch_partition_keys(sph_ctx *c, int64_t m, int n_labels, uint32_t *offsets, uint32_t *dest, uint32_t **order)
 {
-    // dest[k] = position of list entry k in the label-segmented order (a SCATTER map: the caller
-    // then reads the list and the records in list order, which is sector-friendly, and writes
-    // n_labels sequential streams -- the gather form re-read every sector once per label)
+    uint32_t *key = c->alt_keys, *key_out = c->alt_vals, *val_out = c->s_comm_hash;  // scratch (stream-ordered)
+    if (order) *order = val_out;
     if (m == 0) {
         SPH_CUDA_TRY(c, cudaMemsetAsync(offsets, 0, sizeof(uint32_t) * (n_labels + 1), c->stream));
         return SPH_OK;
     }
-    uint32_t *key = c->alt_keys, *key_out = c->alt_vals, *val_out = c->s_comm_hash;  // scratch (stream-ordered)
     const int64_t tiles = (m + kSortTile - 1) / kSortTile;
     SPH_CUDA_TRY(c, cudaMemsetAsync(c->hist, 0, sizeof(uint32_t) * kRadix, c->stream));
     SPH_CUDA_TRY(c, cudaMemsetAsync(c->tile_counter, 0, sizeof(uint32_t), c->stream));
     SPH_CUDA_TRY(c, cudaMemsetAsync(c->tile_status, 0, sizeof(uint32_t) * (size_t)tiles * kRadix, c->stream));
-    gather_label_kernel<<<div_up(m, 256), 256, 0, c->stream>>>(m, ids, label, key);
-    SPH_CHECK_LAUNCH(c);
     int hb = (int)min((int64_t)c->num_sms * 8, (m + 1023) / 1024);
     if (hb < 1) hb = 1;
     radix_hist_kernel<1><<<hb, 256, 0, c->stream>>>(m, key, c->hist);
     SPH_CHECK_LAUNCH(c);
     radix_hist_scan_kernel<<<1, kRadix, 0, c->stream>>>(c->hist);
     SPH_CHECK_LAUNCH(c);
-    segment_offsets_kernel<<<1, 64, 0, c->stream>>>(c->hist, n_labels, (uint32_t)m, offsets);
+    segment_offsets_kernel<<<1, 512, 0, c->stream>>>(c->hist, n_labels, (uint32_t)m, offsets);
     SPH_CHECK_LAUNCH(c);
     {
         int rc = sort_smem_opt_in(c);
         if (rc != SPH_OK) return rc;
     }
-    // values = the implicit list indices 0..m-1 (FIRST), so inv_out[k] is entry k's destination
+    // values = the implicit indices 0..m-1 (FIRST), so inv_out[k] is index k's destination
     onesweep_kernel<true><<<(unsigned)tiles, kSortThreads, sizeof(SortSmem), c->stream>>>(
         m, key, nullptr, key_out, val_out, c->hist, c->tile_status, c->tile_counter, 0, dest);
     SPH_CHECK_LAUNCH(c);
     return SPH_OK;
+}
+
+int launch_partition_by_label(sph_ctx *c, int64_t m, const uint32_t *ids, const int32_t *label, int n_labels,
+                              uint32_t *offsets, uint32_t *dest)
+{
+    // dest[k] = position of list entry k in the label-segmented order (a SCATTER map: the caller
+    // then reads the list and the records in list order, which is sector-friendly, and writes
+    // n_labels sequential streams -- the gather form re-read every sector once per label)
+    if (m > 0) {
+        gather_label_kernel<<<div_up(m, 256), 256, 0, c->stream>>>(m, ids, label, c->alt_keys);
+        SPH_CHECK_LAUNCH(c);
+    }
+    return launch_partition_keys(c, m, n_labels, offsets, dest, nullptr);
 }
 
 // --------------------------------------------------------------------------- generic scan

@@ -137,6 +137,8 @@ int launch_integrate(sph_ctx *c, int64_t n, float dt, const sph_state *in, const
                      const uint32_t *scatter_perm /* NULL = elementwise */);
 int launch_partition_by_label(sph_ctx *c, int64_t m, const uint32_t *ids, const int32_t *label, int n_labels,
                               uint32_t *offsets, uint32_t *dest /* [m] scatter map */);
+int launch_partition_keys(sph_ctx *c, int64_t m, int n_labels /* keys in c->alt_keys, < 256 */, uint32_t *offsets,
+                          uint32_t *dest /* optional */, uint32_t **order /* out: indices in partition order */);
 int launch_scatter_records(sph_ctx *c, int64_t m, const uint32_t *ids, const uint32_t *dest,
                            const sph_state *in, const sph_state *out, uint32_t *packed_ids);
 int launch_balance(sph_ctx *c, int64_t n, const float *posm, int32_t *owner, const int32_t *ptype, int n_types,
