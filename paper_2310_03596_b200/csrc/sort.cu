@@ -22,9 +22,12 @@ __device__ __forceinline__ void hist_add4(uint32_t (*s_hist)[kRadix], const uint
 {
     const uint32_t d0 = (v.x >> (P * kRadixBits)) & (kRadix - 1), d1 = (v.y >> (P * kRadixBits)) & (kRadix - 1);
     const uint32_t d2 = (v.z >> (P * kRadixBits)) & (kRadix - 1), d3 = (v.w >> (P * kRadixBits)) & (kRadix - 1);
-    if (P == 0) {  // the lowest digit changes every few keys: no aggregation pays
-        atomicAdd(&s_hist[P][d0], 1u); atomicAdd(&s_hist[P][d1], 1u);
-        atomicAdd(&s_hist[P][d2], 1u); atomicAdd(&s_hist[P][d3], 1u);
+    if (P == 0) {  // the lowest digit changes every few keys: runs inside the thread's own 4 keys
+        const bool r01 = d1 == d0, r12 = d2 == d1, r23 = d3 == d2;
+        atomicAdd(&s_hist[P][d0], 1u + (r01 ? 1u + (r12 ? 1u + (r23 ? 1u : 0u) : 0u) : 0u));
+        if (!r01) atomicAdd(&s_hist[P][d1], 1u + (r12 ? 1u + (r23 ? 1u : 0u) : 0u));
+        if (!r12) atomicAdd(&s_hist[P][d2], 1u + (r23 ? 1u : 0u));
+        if (!r23) atomicAdd(&s_hist[P][d3], 1u);
         return;
     }
     const bool same = (d0 == d1) & (d2 == d3) & (d0 == d2);
@@ -42,9 +45,15 @@ __device__ __forceinline__ void hist_add4(uint32_t (*s_hist)[kRadix], const uint
 
 template <int NP>
 __global__ void __launch_bounds__(256) radix_hist_kernel(int64_t n, const uint32_t *__restrict__ keys,
-                                                         uint32_t *__restrict__ hist)
+                                                         uint32_t *__restrict__ hist, uint32_t *__restrict__ status,
+                                                         int64_t n_status, uint32_t *__restrict__ tickets, int n_tickets)
 {
     __shared__ uint32_t s_hist[kMaxPasses][kRadix];
+    // the look-back status words and tile tickets of the passes are cleared here (this kernel only
+    // reads otherwise, the stores ride along): two memset launches less per sort
+    for (int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; i < n_status; i += (int64_t)gridDim.x * blockDim.x)
+        status[i] = 0u;
+    if (blockIdx.x == 0 && threadIdx.x < n_tickets) tickets[threadIdx.x] = 0u;
     for (int i = threadIdx.x; i < kMaxPasses * kRadix; i += blockDim.x) (&s_hist[0][0])[i] = 0;
     __syncthreads();
     const int lane = threadIdx.x & 31;
@@ -134,7 +143,7 @@ struct SortSmem {
 };
 
 template <bool FIRST>
-__global__ void __launch_bounds__(kSortThreads, 2)
+__global__ void __launch_bounds__(kSortThreads, 3)
 onesweep_kernel(int64_t n, const uint32_t *__restrict__ keys_in, const uint32_t *__restrict__ vals_in,
                 uint32_t *__restrict__ keys_out, uint32_t *__restrict__ vals_out,
                 const uint32_t *__restrict__ hist_excl, uint32_t *status, uint32_t *ticket, int shift,
@@ -327,16 +336,14 @@ int launch_sort(sph_ctx *c, int64_t n, const uint32_t *hash, uint32_t *sorted_ha
     }
     const int64_t tiles = (n + kSortTile - 1) / kSortTile;
     SPH_CUDA_TRY(c, cudaMemsetAsync(c->hist, 0, sizeof(uint32_t) * kMaxPasses * kRadix, c->stream));
-    SPH_CUDA_TRY(c, cudaMemsetAsync(c->tile_counter, 0, sizeof(uint32_t) * (kMaxPasses + 2), c->stream));
-    SPH_CUDA_TRY(c, cudaMemsetAsync(c->tile_status, 0, sizeof(uint32_t) * (size_t)P * tiles * kRadix,
-                                    c->stream));
+    const int64_t n_status = (int64_t)P * tiles * kRadix;
     int hb = (int)min((int64_t)c->num_sms * 8, (n + 1023) / 1024);
     if (hb < 1) hb = 1;
     switch (P) {
-    case 1: radix_hist_kernel<1><<<hb, 256, 0, c->stream>>>(n, hash, c->hist); break;
-    case 2: radix_hist_kernel<2><<<hb, 256, 0, c->stream>>>(n, hash, c->hist); break;
-    case 3: radix_hist_kernel<3><<<hb, 256, 0, c->stream>>>(n, hash, c->hist); break;
-    default: radix_hist_kernel<4><<<hb, 256, 0, c->stream>>>(n, hash, c->hist); break;
+    case 1: radix_hist_kernel<1><<<hb, 256, 0, c->stream>>>(n, hash, c->hist, c->tile_status, n_status, c->tile_counter, kMaxPasses); break;
+    case 2: radix_hist_kernel<2><<<hb, 256, 0, c->stream>>>(n, hash, c->hist, c->tile_status, n_status, c->tile_counter, kMaxPasses); break;
+    case 3: radix_hist_kernel<3><<<hb, 256, 0, c->stream>>>(n, hash, c->hist, c->tile_status, n_status, c->tile_counter, kMaxPasses); break;
+    default: radix_hist_kernel<4><<<hb, 256, 0, c->stream>>>(n, hash, c->hist, c->tile_status, n_status, c->tile_counter, kMaxPasses); break;
     }
     SPH_CHECK_LAUNCH(c);
     radix_hist_scan_kernel<<<P, kRadix, 0, c->stream>>>(c->hist);
@@ -401,11 +408,9 @@ int launch_partition_keys(sph_ctx *c, int64_t m, int n_labels, uint32_t *offsets
     }
     const int64_t tiles = (m + kSortTile - 1) / kSortTile;
     SPH_CUDA_TRY(c, cudaMemsetAsync(c->hist, 0, sizeof(uint32_t) * kRadix, c->stream));
-    SPH_CUDA_TRY(c, cudaMemsetAsync(c->tile_counter, 0, sizeof(uint32_t), c->stream));
-    SPH_CUDA_TRY(c, cudaMemsetAsync(c->tile_status, 0, sizeof(uint32_t) * (size_t)tiles * kRadix, c->stream));
     int hb = (int)min((int64_t)c->num_sms * 8, (m + 1023) / 1024);
     if (hb < 1) hb = 1;
-    radix_hist_kernel<1><<<hb, 256, 0, c->stream>>>(m, key, c->hist);
+    radix_hist_kernel<1><<<hb, 256, 0, c->stream>>>(m, key, c->hist, c->tile_status, tiles * kRadix, c->tile_counter, 1);
     SPH_CHECK_LAUNCH(c);
     radix_hist_scan_kernel<<<1, kRadix, 0, c->stream>>>(c->hist);
     SPH_CHECK_LAUNCH(c);

@@ -14,7 +14,7 @@ constexpr int kRadix = 1 << kRadixBits;
 constexpr int kMaxPasses = 4;
 
 // onesweep tile geometry
-constexpr int kSortThreads = 512;
+constexpr int kSortThreads = 384;
 constexpr int kSortItems = 16;
 constexpr int kSortTile = kSortThreads * kSortItems;  // 8192 keys per tile
 
