@@ -99,12 +99,12 @@ __device__ __forceinline__ void mbar_wait(uint64_t *bar, uint32_t parity)
         "{\n"
         ".reg .pred p;\n"
         "WAIT_%=:\n"
-        "mbarrier.try_wait.parity.shared::cta.b64 p, [%0], %1;\n"
+        "mbarrier.try_wait.parity.shared::cta.b64 p, [%0], %1, %2;\n"
         "@p bra DONE_%=;\n"
         "bra WAIT_%=;\n"
         "DONE_%=:\n"
         "}\n" ::"r"(smem_u32(bar)),
-        "r"(parity)
+        "r"(parity), "r"(0x989680u)   // suspend-time hint: the warp sleeps until the phase completes
         : "memory");
 }
 __device__ __forceinline__ void tma_load_1d(void *dst, const void *src, uint32_t bytes, uint64_t *bar)
@@ -208,6 +208,23 @@ interact_tiled_kernel(Packed rec, InteractIn in, const uint32_t *__restrict__ cs
         const int lo = (int)cs[rrow + max(cx0 - 1, 0)], hi = (int)ce[rrow + min(cx0 + nbx, g.nx - 1)];
         if (hi > lo) { run_lo = lo; run_len = hi - lo; }
     }
+    // stencil rows of bucket b = warp (candidate table below): lane r' < 9 looks up stencil row
+    // r' = (dy + 1) + 3 (dz + 1).  Issued here so that every global load of the tile set-up is in
+    // flight at once (one round trip instead of three).
+    int rowq_sg = 0, rowq_len = 0;
+    {
+        const int bx_ = warp % kTBX, by_ = warp / kTBX;
+        if (lane < 9 && bx_ < nbx && by_ < nby) {
+            const int wr = (by_ + lane % 3) + kRowsY * (lane / 3);
+            const int y = cy0 - 1 + (wr % kRowsY), z = cz - 1 + (wr / kRowsY);
+            if (y >= 0 && y < g.ny && z >= 0 && z < g.nz) {
+                const uint32_t row = (uint32_t)g.nx * ((uint32_t)y + (uint32_t)g.ny * (uint32_t)z);
+                const int cxb_ = cx0 + bx_;
+                rowq_sg = (int)cs[row + max(cxb_ - 1, 0)];
+                rowq_len = max((int)ce[row + min(cxb_ + 1, g.nx - 1)] - rowq_sg, 0);
+            }
+        }
+    }
     const int run_cnt = run_len;
     int run_off = run_cnt;                   // exclusive prefix over lanes 0..kRuns-1
 #pragma unroll
@@ -265,18 +282,8 @@ interact_tiled_kernel(Packed rec, InteractIn in, const uint32_t *__restrict__ cs
         //      shifted so that (table position) == (record index) mod 8.  Lane r' < 9 looks up
         //      stencil row r' = (dy + 1) + 3 (dz + 1), i.e. window run (by + r' % 3) + kRowsY (r' / 3).
         {
-            int s_r = 0, len_r = 0;
-            if (nt > 0 && lane < 9) {
-                const int wr = (by + lane % 3) + kRowsY * (lane / 3);
-                const int y = cy0 - 1 + (wr % kRowsY), z = cz - 1 + (wr / kRowsY);
-                if (y >= 0 && y < g.ny && z >= 0 && z < g.nz) {
-                    const uint32_t row = (uint32_t)g.nx * ((uint32_t)y + (uint32_t)g.ny * (uint32_t)z);
-                    const int sg = (int)cs[row + max(cxb - 1, 0)], eg = (int)ce[row + min(cxb + 1, g.nx - 1)];
-                    len_r = max(eg - sg, 0);
-                    // offset of the stencil row inside window run wr (held by lane wr)
-                    s_r = sg;
-                }
-            }
+            int s_r = rowq_sg;   // (loaded at the top of the kernel, together with the run descriptors)
+            const int len_r = nt > 0 ? rowq_len : 0;
             // window run descriptors of the 9 rows (every lane fetches the one of its row)
             const int wr_l = (lane < 9) ? (by + lane % 3) + kRowsY * (lane / 3) : 0;
             const int w_off = __shfl_sync(0xffffffffu, run_off, wr_l);
