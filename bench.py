@@ -44,7 +44,10 @@ BYTES_PER_PARTICLE = {   # algorithmic HBM bytes per particle per stage (DESIGN.
 }
 # dram__bytes_read.sum + dram__bytes_write.sum per launch of the interaction kernel from the
 # committed `ncu --set full` capture (profiles/), keyed by config; None until captured.
-NCU_TRAFFIC_BYTES = {1: 93.69e6}   # profiles/r01d_interact_v6_ncu_full.md (68.6 MB read + 25.1 MB written)
+NCU_TRAFFIC_BYTES = {
+    1: 93.69e6,    # profiles/r01d_interact_v6_ncu_full.md (68.6 MB read + 25.1 MB written)
+    4: 12.302e9,   # profiles/r02a_interact_cfg4_ncu_full.md (8.636 GB read + 3.666 GB written; 6.14 GB algorithmic)
+}
 
 
 def load_peaks():

@@ -122,6 +122,17 @@ __device__ __forceinline__ f32x2 fma2(f32x2 a, f32x2 b, f32x2 c)
     asm("fma.rn.f32x2 %0, %1, %2, %3;" : "=l"(d) : "l"(a), "l"(b), "l"(c));
     return d;
 }
+// in-place accumulate forms (acc += a * b, acc += a): the read-modify-write of one PTX register
+// keeps ptxas from ping-ponging the accumulators between two register sets (it closed the loop
+// of phase 2 with 14 moves per round before)
+__device__ __forceinline__ void fma2_acc(f32x2 &acc, f32x2 a, f32x2 b)
+{
+    asm("fma.rn.f32x2 %0, %1, %2, %0;" : "+l"(acc) : "l"(a), "l"(b));
+}
+__device__ __forceinline__ void add2_acc(f32x2 &acc, f32x2 a)
+{
+    asm("add.rn.f32x2 %0, %0, %1;" : "+l"(acc) : "l"(a));
+}
 __device__ __forceinline__ f32x2 mul2(f32x2 a, f32x2 b)
 {
     f32x2 d;
@@ -191,19 +202,19 @@ struct PairAccum2 {
         const float mz = lo_of(mwz), wz = hi_of(mwz);
         const f32x2 dvxy = sub2(pk(pb.x, pb.y), tvxy);
         const float dvz = pb.z - tvz;
-        dr2 = fma2(dvxy, mxy, dr2);
+        fma2_acc(dr2, dvxy, mxy);
         drz = fmaf(dvz, mz, drz);
-        Lx = fma2(bc(lo_of(dvxy)), wxy, Lx);
-        Ly = fma2(bc(hi_of(dvxy)), wxy, Ly);
-        Lz = fma2(bc(dvz), wxy, Lz);
-        Lc = fma2(bc(wz), dvxy, Lc);
+        fma2_acc(Lx, bc(lo_of(dvxy)), wxy);
+        fma2_acc(Ly, bc(hi_of(dvxy)), wxy);
+        fma2_acc(Lz, bc(dvz), wxy);
+        fma2_acc(Lc, bc(wz), dvxy);
         Lzz = fmaf(dvz, wz, Lzz);
-        g2 = add2(g2, mxy);
+        add2_acc(g2, mxy);
         gz += mz;
-        a2 = fma2(bc(lo_of(mxy)), pk(pc.x, pc.y), a2);
-        a2 = fma2(bc(hi_of(mxy)), pk(VH ? pc.y : pc.z, pc.w), a2);
-        a2 = fma2(bc(mz), pk(pd.x, pd.y), a2);
-        az2 = fma2(pk(pd.x, pd.y), mxy, az2);
+        fma2_acc(a2, bc(lo_of(mxy)), pk(pc.x, pc.y));
+        fma2_acc(a2, bc(hi_of(mxy)), pk(VH ? pc.y : pc.z, pc.w));
+        fma2_acc(a2, bc(mz), pk(pd.x, pd.y));
+        fma2_acc(az2, pk(pd.x, pd.y), mxy);
         azz = fmaf(pb.w, mz, azz);
         return r2;
     }
