@@ -387,6 +387,26 @@ def test_balance_sweep_matches_oracle_bit_exact(sph, oracle, make, g):
     ctx.close()
 
 
+@pytest.mark.parametrize("hmax", [1, 5, 37])
+def test_balance_tie_heavy_small_hmax(sph, oracle, hmax):
+    """Few hash values (hmax = 1, 5, 37 on 46 k particles): thousands of particles share the
+    threshold hash of every pair, so the id-ordered choice among the ties (reading B6; a three-level
+    radix select on the id in the kernel, a sort in the oracle) decides almost every swap."""
+    w = wl.lattice_block(40, 36, 32, 0.1, 29, owners=("random", 4))
+    ctx = sph.Context.for_workload(w)
+    posm = torch.from_numpy(w.posm).cuda()
+    own_gpu = torch.from_numpy(w.owner.copy()).cuda()
+    own_ref = w.owner.copy()
+    for sweep in range(2):
+        bh, sw = ctx.sph_balance(posm, own_gpu, hmax=hmax)
+        torch.cuda.synchronize()
+        own_ref, k, bh_ref = oracle.balance(w.posm, own_ref, 4, hmax=hmax)
+        assert int(sw.cpu()[0]) == k and (sweep > 0 or k > 0), sweep
+        np.testing.assert_array_equal(bh.cpu().numpy(), bh_ref, err_msg=f"bal_hash sweep {sweep}")
+        np.testing.assert_array_equal(own_gpu.cpu().numpy(), own_ref, err_msg=f"owner sweep {sweep}")
+    ctx.close()
+
+
 @pytest.mark.parametrize("g,nt,alpha", [(3, 2, 0.1), (5, 3, 0.1), (4, 2, 1.0), (4, 1, 0.0)])
 def test_balance_types_matches_oracle_bit_exact(sph, oracle, g, nt, alpha):
     """sph_balance_types (Cg' = alpha Cg_all + (1 - alpha) Cg_type) against

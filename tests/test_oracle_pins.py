@@ -695,6 +695,59 @@ def test_balance_hash_against_independent_projection():
             assert bh[side & moved].min() >= bh[side & ~moved].max()
 
 
+def test_balance_hash_exact_rational_arithmetic_and_tie_order():
+    """Readings B2-B4 and B6 pinned by exact arithmetic.  Positions on the 2^-6 dyadic grid are exact
+    in the 2^-16 fixed point of B2, so the centres of gravity are exact rationals; the projection s
+    and hmax (2 s - 1) are evaluated with fractions.Fraction (no rounding at all) and the oracle's
+    fp64 hash must equal the exact ceil() for EVERY particle whose exact value is not within 1e-9
+    of an integer.  The coarse grid also produces many equal hashes: the n movers of a side must be
+    the first n of that side in the order (hash descending, id ascending) -- reading B6 -- which is
+    recomputed here with a plain sort."""
+    from fractions import Fraction as Fr
+    import math
+    for hmax, seed in ((1000, 17), (6, 18)):        # hmax = 6: six hash values only -> ties everywhere
+        rng = np.random.default_rng(seed)
+        n = 240
+        xi = rng.integers(0, 8 * 64, size=(n, 3))              # multiples of 2^-6 in [0, 8)
+        posm = np.ones((n, 4), np.float32)
+        posm[:, :3] = (xi / 64.0).astype(np.float32)
+        own0 = (rng.random(n) < 0.45).astype(np.int32)
+        own, k, bh = orc.balance(posm, own0, 2, hmax=hmax)
+        X = [[Fr(int(v), 64) for v in row] for row in xi]
+        cg = []
+        for g in (0, 1):
+            ids = [i for i in range(n) if own0[i] == g]
+            cg.append([sum(X[i][a] for i in ids) / len(ids) for a in range(3)])
+        exact = np.zeros(n, np.int64)
+        near_integer = np.zeros(n, bool)
+        for i in range(n):
+            g = int(own0[i])
+            d = [cg[1 - g][a] - cg[g][a] for a in range(3)]
+            s = sum((X[i][a] - cg[g][a]) * d[a] for a in range(3)) / sum(da * da for da in d)
+            if s >= 1:
+                exact[i] = hmax
+            elif s > Fr(1, 2):
+                v = hmax * (2 * s - 1)
+                exact[i] = min(max(math.ceil(v), 1), hmax)
+                near_integer[i] = abs(v - round(v)) < Fr(1, 10 ** 9)
+        ok = ~near_integer
+        assert ok.sum() >= n - 2
+        np.testing.assert_array_equal(bh[ok], exact[ok])
+        # B6: the movers of each side are the first n_move in (hash descending, id ascending)
+        pos = [np.nonzero((own0 == g) & (bh > 0))[0] for g in (0, 1)]
+        n_move = min(len(pos[0]), len(pos[1]))
+        assert k == n_move and n_move > 0
+        for g in (0, 1):
+            order = sorted(pos[g].tolist(), key=lambda i: (-int(bh[i]), i))
+            assert set(np.nonzero((own != own0) & (own0 == g))[0].tolist()) == set(order[:n_move])
+        if hmax == 6:
+            # the side that keeps some of its positive hashes cuts INSIDE a group of equal hashes,
+            # so the id order decides who moves
+            g = 0 if len(pos[0]) > len(pos[1]) else 1
+            order = sorted(pos[g].tolist(), key=lambda i: (-int(bh[i]), i))
+            assert n_move < len(order) and bh[order[n_move - 1]] == bh[order[n_move]]
+
+
 def test_balance_restores_a_compact_decomposition():
     """The Fig. 1 -> Fig. 2 effect (PAPER.md:38 'the information exchange subset is always close
     to a surface'): random labels make every particle a boundary particle; a few sweeps bring the
