@@ -22,6 +22,9 @@
  *  - Return value: 0 = SPH_OK, negative = error (below).  No exception crosses this boundary.
  *  - Per-particle arrays: posm [n][4] = x, y, z, m;  velr [n][4] = vx, vy, vz, rho;
  *    sig[c] [n], c = xx, yy, zz, xy, xz, yz (SoA);  owner [n] in [0, n_owners).
+ *    The labels are the caller's contract and are NOT validated on the device (a check would
+ *    cost a pass and a host synchronisation): the kernels use label & 31 (bucket masks) and
+ *    label & 255 (partition passes), so an out-of-range label gives wrong boundary sets, never a fault.
  *    All real data fp32, all hashes / indices uint32.  posm / velr / acc must be 16-byte aligned,
  *    everything else 4-byte aligned.
  *  - "sorted position k": index in the (hash, id) order produced by sph_sort; perm[k] is the
