@@ -253,7 +253,9 @@ int sph_step_varh(sph_ctx *ctx, int64_t n, float dt, const sph_state *state, con
 /* End-to-end variant with HOST buffers (pinned memory recommended): uploads the id-ordered state,
  * runs `steps` iterations, downloads the state, the boundary list of the last step and the
  * counters, and synchronises the stream before returning.  Device staging lives in the ctx
- * (allocated on first use).  host_state pointers are host; boundary_ids host capacity n (may be
+ * (allocated on first use).  posm goes up first on the ctx's stream, the rest of the state on a
+ * second stream owned by the ctx while hash + sort already run; the download follows the last
+ * step (its epilogue writes the whole state, so nothing of it can leave earlier).  host_state pointers are host; boundary_ids host capacity n (may be
  * NULL); boundary_count / pair_count host scalars (may be NULL; pair_count accumulates over the
  * steps). */
 int sph_step_host(sph_ctx *ctx, int64_t n, float dt, int32_t steps, const sph_state *host_state,

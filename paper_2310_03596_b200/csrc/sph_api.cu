@@ -131,6 +131,8 @@ int sph_create(sph_ctx **out, const sph_params *p, int64_t max_n, void *cuda_str
     c->launches = 0;
     c->last_err = cudaSuccess;
     c->staging_ready = false;
+    c->host_streams_ready = false;
+    c->wait_before_reorder = nullptr;
     c->rec_fresh = false;
     c->attr_sort = c->attr_interact = false;
     memset(&c->staging, 0, sizeof(c->staging));
@@ -176,6 +178,12 @@ int sph_destroy(sph_ctx *c)
             for (int i = 0; i < 9; ++i) cudaEventDestroy(c->timing.ev[s][i]);
     if (c->staging_ready) {
         cudaFree(c->staging.posm);
+    }
+    if (c->host_streams_ready) {
+        cudaStreamSynchronize(c->copy_stream);
+        cudaEventDestroy(c->ev_posm);
+        cudaEventDestroy(c->ev_rest);
+        cudaStreamDestroy(c->copy_stream);
     }
     cudaFree(c->arena);
     delete c;
@@ -328,6 +336,10 @@ static int step_impl(sph_ctx *c, int64_t n, float dt, const sph_state *state, ui
     t.mark();
     if ((rc = launch_sort(c, n, hash, sorted_hash, perm)) != SPH_OK) return rc;
     t.mark();
+    if (c->wait_before_reorder) {   // sph_step_host: the rest of the state arrives on the copy stream
+        SPH_CUDA_TRY(c, cudaStreamWaitEvent(c->stream, c->wait_before_reorder, 0));
+        c->wait_before_reorder = nullptr;
+    }
     if ((rc = launch_reorder(c, n, perm, state, &c->sorted, hp, c->sorted_h)) != SPH_OK) return rc;
     t.mark();
     if ((rc = launch_cell_ranges(c, n, sorted_hash, cell_start, cell_end)) != SPH_OK) return rc;
@@ -403,16 +415,34 @@ int sph_step_host(sph_ctx *c, int64_t n, float dt, int32_t steps, const sph_stat
     const sph_state &d = c->staging;
     cudaStream_t s = c->stream;
     const size_t nn = (size_t)n;
+    if (!c->host_streams_ready) {
+        SPH_CUDA_TRY(c, cudaStreamCreateWithFlags(&c->copy_stream, cudaStreamNonBlocking));
+        SPH_CUDA_TRY(c, cudaEventCreateWithFlags(&c->ev_posm, cudaEventDisableTiming));
+        SPH_CUDA_TRY(c, cudaEventCreateWithFlags(&c->ev_rest, cudaEventDisableTiming));
+        c->host_streams_ready = true;
+    }
+    // posm first, on the ctx's stream: hash, sort and nothing else of the step can start on it.
+    // The other 44 bytes per particle follow on the copy stream (behind posm, so that the two
+    // uploads do not share the link), and the step waits for them in front of its reorder pass.
+    cudaStream_t s2 = c->copy_stream;
     SPH_CUDA_TRY(c, cudaMemcpyAsync(d.posm, hs->posm, 16 * nn, cudaMemcpyHostToDevice, s));
-    SPH_CUDA_TRY(c, cudaMemcpyAsync(d.velr, hs->velr, 16 * nn, cudaMemcpyHostToDevice, s));
+    SPH_CUDA_TRY(c, cudaEventRecord(c->ev_posm, s));
+    SPH_CUDA_TRY(c, cudaStreamWaitEvent(s2, c->ev_posm, 0));
+    SPH_CUDA_TRY(c, cudaMemcpyAsync(d.velr, hs->velr, 16 * nn, cudaMemcpyHostToDevice, s2));
     for (int i = 0; i < 6; ++i)
-        SPH_CUDA_TRY(c, cudaMemcpyAsync(d.sig[i], hs->sig[i], 4 * nn, cudaMemcpyHostToDevice, s));
-    SPH_CUDA_TRY(c, cudaMemcpyAsync(d.owner, hs->owner, 4 * nn, cudaMemcpyHostToDevice, s));
+        SPH_CUDA_TRY(c, cudaMemcpyAsync(d.sig[i], hs->sig[i], 4 * nn, cudaMemcpyHostToDevice, s2));
+    SPH_CUDA_TRY(c, cudaMemcpyAsync(d.owner, hs->owner, 4 * nn, cudaMemcpyHostToDevice, s2));
+    SPH_CUDA_TRY(c, cudaEventRecord(c->ev_rest, s2));
+    c->wait_before_reorder = c->ev_rest;
     SPH_CUDA_TRY(c, cudaMemsetAsync(c->s_pair_count, 0, 2 * sizeof(unsigned long long), s));
     for (int32_t it = 0; it < steps; ++it) {
         int rc = step_impl(c, n, dt, &d, nullptr, nullptr, nullptr, nullptr, nullptr, nullptr, nullptr,
                            nullptr, nullptr, nullptr, nullptr, nullptr, c->s_pair_count, false);
-        if (rc != SPH_OK) return rc;
+        if (rc != SPH_OK) { c->wait_before_reorder = nullptr; cudaStreamSynchronize(s2); return rc; }
+    }
+    if (c->wait_before_reorder) {   // steps == 0: nothing has waited for the second upload yet
+        SPH_CUDA_TRY(c, cudaStreamWaitEvent(s, c->wait_before_reorder, 0));
+        c->wait_before_reorder = nullptr;
     }
     SPH_CUDA_TRY(c, cudaMemcpyAsync(hs->posm, d.posm, 16 * nn, cudaMemcpyDeviceToHost, s));
     SPH_CUDA_TRY(c, cudaMemcpyAsync(hs->velr, d.velr, 16 * nn, cudaMemcpyDeviceToHost, s));

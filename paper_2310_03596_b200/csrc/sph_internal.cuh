@@ -67,6 +67,12 @@ struct sph_ctx {
     int n_passes;
     int64_t launches;
     cudaError_t last_err;
+    // sph_step_host: a second stream uploads velr / sig / owner while hash + sort (which need posm
+    // only) already run; step_impl waits for `wait_before_reorder` (if set) before the reorder pass
+    cudaStream_t copy_stream;
+    cudaEvent_t ev_posm, ev_rest;
+    bool host_streams_ready;
+    cudaEvent_t wait_before_reorder;
 
     // ---- scratch (device) ----
     void *arena;                 // one allocation, carved below
