@@ -210,6 +210,32 @@ def test_step_host_end_to_end(sph, oracle):
     ctx.close()
 
 
+def test_step_host_two_streams_steps0_repeat_and_multistep(sph, oracle):
+    """sph_step_host uploads posm on the ctx's stream and the rest of the state on a second one:
+    steps = 0 must hand the state back bit for bit (the download has to wait for BOTH uploads),
+    two calls of one step equal one call of two steps bit for bit (the staging is reused), and
+    the two-step result matches the oracle run in lock-step."""
+    w = wl.t1b(side=14, seed=1112)
+    ctx = sph.Context.for_workload(w)
+    host = sph.State.from_numpy(w.posm, w.velr, w.sig, w.owner, device="cpu", pin=True)
+    m0, _ = ctx.sph_step_host(host, w.dt, steps=0)
+    assert m0 == 0
+    np.testing.assert_array_equal(host.posm.numpy(), w.posm)
+    np.testing.assert_array_equal(host.velr.numpy(), w.velr)
+    np.testing.assert_array_equal(host.sig.numpy(), w.sig)
+    a = sph.State.from_numpy(w.posm, w.velr, w.sig, w.owner, device="cpu", pin=True)
+    b = sph.State.from_numpy(w.posm, w.velr, w.sig, w.owner, device="cpu", pin=True)
+    ctx.sph_step_host(a, w.dt, steps=1)
+    r1 = oracle.step(w.posm, w.velr, w.sig, w.owner, w.origin, w.dims, w.h, w.K, w.G, w.n_owners, w.dt)
+    parity.compare_state(a, r1)
+    ma, _ = ctx.sph_step_host(a, w.dt, steps=1)
+    mb, _ = ctx.sph_step_host(b, w.dt, steps=2)
+    assert ma == mb
+    for x, y in ((a.posm, b.posm), (a.velr, b.velr), (a.sig, b.sig)):
+        np.testing.assert_array_equal(x.numpy(), y.numpy())
+    ctx.close()
+
+
 def test_error_codes(sph):
     with pytest.raises(sph.SphError):
         sph.Context([0, 0, 0], [0, 1, 1], 1.3, max_n=10)
