@@ -10,9 +10,6 @@
 // the live key bits ceil(log2(cells)) are sorted.  Stability + ascending ids on input give the
 // lexicographic (hash, id) order.
 #include "sph_internal.cuh"
-#ifndef SPH_KLOOK
-#define SPH_KLOOK 4
-#endif
 
 namespace sphb {
 
@@ -294,7 +291,7 @@ onesweep_kernel(int64_t n, const uint32_t *__restrict__ keys_in, const uint32_t 
         if (tile > 0) {
             // kLook status words are requested at once (independent loads), then consumed in
             // order: a thread-serial walk would cost one L2 round trip per preceding tile
-            constexpr int kLook = SPH_KLOOK;   // measured at 64 M keys: 1 -> 1.08 ms, 2 -> 0.99, 4 -> 0.966, 8 -> 0.974, 16 -> 1.02
+            constexpr int kLook = 4;   // measured at 64 M keys: 1 -> 1.08 ms, 2 -> 0.99, 4 -> 0.966, 8 -> 0.974, 16 -> 1.02; with the L2 prefetch: 2 -> 0.905, 4 -> 0.882, 8 -> 0.890; batches that grow to 16 after a fully consumed batch: 0.937 (the walk mostly polls ONE unpublished word: 10.4 round trips per tile and warp)
             int64_t t = (int64_t)tile - 1;
             bool done = false;
             while (!done) {
