@@ -91,10 +91,26 @@ __global__ void __launch_bounds__(256) radix_hist_kernel(int64_t n, const uint32
     n -= head;
     const int64_t n4 = n >> 2;                       // whole 128-bit groups
     const int64_t stride = (int64_t)gridDim.x * blockDim.x;
-    // block-uniform trip count (the warp-collective needs full warps), two loads in flight
-    const int64_t iters = (n4 + 2 * stride - 1) / (2 * stride);
     int64_t g = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
     const uint4 *k4 = reinterpret_cast<const uint4 *>(keys);
+    // main part: iterations in which every thread of the grid has data -- four loads in flight,
+    // no bounds checks, no votes
+    const int64_t full = n4 / (4 * stride);
+    for (int64_t it = 0; it < full; ++it, g += 4 * stride) {
+        const uint4 a = __ldcs(k4 + g), b = __ldcs(k4 + g + stride);
+        const uint4 c = __ldcs(k4 + g + 2 * stride), d = __ldcs(k4 + g + 3 * stride);
+        hist_add4<0>(s_hist, a, lane);
+        if (NP > 1) hist_upper<NP>(s_hist, a, lane);
+        hist_add4<0>(s_hist, b, lane);
+        if (NP > 1) hist_upper<NP>(s_hist, b, lane);
+        hist_add4<0>(s_hist, c, lane);
+        if (NP > 1) hist_upper<NP>(s_hist, c, lane);
+        hist_add4<0>(s_hist, d, lane);
+        if (NP > 1) hist_upper<NP>(s_hist, d, lane);
+    }
+    // rest: block-uniform trip count (the warp-collective needs full warps), two loads in flight
+    const int64_t rest = n4 - full * 4 * stride;
+    const int64_t iters = (rest + 2 * stride - 1) / (2 * stride);
     for (int64_t it = 0; it < iters; ++it, g += 2 * stride) {
         const bool ok0 = g < n4, ok1 = g + stride < n4;
         uint4 a = make_uint4(0, 0, 0, 0), b = a;
