@@ -374,6 +374,8 @@ def run_ours(args, rank, world, local_rank):
             # no separate pass runs, the stage boundary is kept only for the report
             e["fused_into"] = "interact"
             b = None
+        if k_ == "hash":
+            e["note"] = "fused with the digit histograms of the sort inside sph_step (the sort reads its keys once less)"
         if b and k_ != "interact" and v > 0:
             e["gbs"] = round(b * n / (v * 1e-3) / 1e9, 1)
             e["hbm_frac"] = round(e["gbs"] / peaks["hbm_gbs"], 3)

@@ -4,18 +4,6 @@
 
 namespace sphb {
 
-__device__ __forceinline__ uint32_t bucket_coord(float x, float o, float inv, int n)
-{
-    // fp32 sequence pinned by reading S2: sub, mul, floor, clamp (no contraction possible)
-    float t = __fsub_rn(x, o);
-    float u = __fmul_rn(t, inv);
-    float f = floorf(u);
-    float top = (float)(n - 1);
-    f = f < 0.0f ? 0.0f : f;
-    f = f > top ? top : f;
-    return (uint32_t)(int)f;
-}
-
 __global__ void __launch_bounds__(256) hash_kernel(int64_t n, const float4 *__restrict__ posm,
                                                    uint32_t *__restrict__ hash, Grid g)
 {
@@ -26,16 +14,10 @@ __global__ void __launch_bounds__(256) hash_kernel(int64_t n, const float4 *__re
     if (i0 < n) p0 = __ldcs(posm + i0);
     if (i1 < n) p1 = __ldcs(posm + i1);
     if (i0 < n) {
-        uint32_t cx = bucket_coord(p0.x, g.ox, g.inv_edge, g.nx);
-        uint32_t cy = bucket_coord(p0.y, g.oy, g.inv_edge, g.ny);
-        uint32_t cz = bucket_coord(p0.z, g.oz, g.inv_edge, g.nz);
-        hash[i0] = cx + (uint32_t)g.nx * (cy + (uint32_t)g.ny * cz);
+        hash[i0] = bucket_hash(p0, g);
     }
     if (i1 < n) {
-        uint32_t cx = bucket_coord(p1.x, g.ox, g.inv_edge, g.nx);
-        uint32_t cy = bucket_coord(p1.y, g.oy, g.inv_edge, g.ny);
-        uint32_t cz = bucket_coord(p1.z, g.oz, g.inv_edge, g.nz);
-        hash[i1] = cx + (uint32_t)g.nx * (cy + (uint32_t)g.ny * cz);
+        hash[i1] = bucket_hash(p1, g);
     }
 }
 

@@ -145,6 +145,58 @@ __global__ void __launch_bounds__(256) radix_hist_kernel(int64_t n, const uint32
     }
 }
 
+// Stage 1 + the histogram of stage 2 in ONE pass over the positions (inside sph_step): the bucket
+// hash of PAPER.md:13 / :19 (readings S1-S3, the pinned fp32 sequence of bucket_hash) is written and
+// counted while it is still in registers, so the sort reads its keys once less (4 of its 52 bytes
+// per particle and a 60 us kernel at 64 M particles).  A warp takes 128 consecutive ids per
+// iteration (four coalesced 16-byte loads per lane); the digit counts follow the histogram kernel
+// above: plain increments for the lowest digit, one match for all upper digits.
+template <int NP>
+__global__ void __launch_bounds__(256) hash_hist_kernel(int64_t n, const float4 *__restrict__ posm,
+                                                        uint32_t *__restrict__ hash, Grid g,
+                                                        uint32_t *__restrict__ hist, uint32_t *__restrict__ status,
+                                                        int64_t n_status, uint32_t *__restrict__ tickets, int n_tickets)
+{
+    __shared__ uint32_t s_hist[kMaxPasses][kRadix];
+    for (int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; i < n_status; i += (int64_t)gridDim.x * blockDim.x)
+        status[i] = 0u;
+    if (blockIdx.x == 0 && threadIdx.x < n_tickets) tickets[threadIdx.x] = 0u;
+    for (int i = threadIdx.x; i < kMaxPasses * kRadix; i += blockDim.x) (&s_hist[0][0])[i] = 0;
+    __syncthreads();
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    const int64_t chunk = 256 * 4;                       // particles per block and iteration
+    for (int64_t base = (int64_t)blockIdx.x * chunk; base < n; base += (int64_t)gridDim.x * chunk) {
+        const int64_t i0 = base + warp * 128 + lane;
+        {   // the warp's 16 lines of the next iteration go to the L2 while this one is processed
+            const int64_t nb = base + (int64_t)gridDim.x * chunk + warp * 128 + lane * 8;
+            if (lane < 16 && nb < n) asm volatile("prefetch.global.L2 [%0];" ::"l"(posm + nb));
+        }
+        if (base + chunk <= n) {                          // block-uniform: every lane has four particles
+            const float4 p0 = __ldcs(posm + i0), p1 = __ldcs(posm + i0 + 32);
+            const float4 p2 = __ldcs(posm + i0 + 64), p3 = __ldcs(posm + i0 + 96);
+            uint4 v;
+            v.x = bucket_hash(p0, g); v.y = bucket_hash(p1, g); v.z = bucket_hash(p2, g); v.w = bucket_hash(p3, g);
+            hash[i0] = v.x; hash[i0 + 32] = v.y; hash[i0 + 64] = v.z; hash[i0 + 96] = v.w;
+            hist_add4<0>(s_hist, v, lane);
+            if (NP > 1) hist_upper<NP>(s_hist, v, lane);
+        } else {
+            for (int j = 0; j < 4; ++j) {
+                const int64_t i = i0 + 32 * j;
+                if (i < n) {
+                    const uint32_t k = bucket_hash(__ldcs(posm + i), g);
+                    hash[i] = k;
+                    for (int p = 0; p < NP; ++p) atomicAdd(&s_hist[p][(k >> (p * kRadixBits)) & (kRadix - 1)], 1u);
+                }
+            }
+        }
+    }
+    __syncthreads();
+    for (int i = threadIdx.x; i < NP * kRadix; i += blockDim.x) {
+        uint32_t v = (&s_hist[0][0])[i];
+        if (v) atomicAdd(hist + i, v);
+    }
+}
+
 // exclusive scan of each pass's 256-bin histogram, in place; one block per pass
 __global__ void __launch_bounds__(kRadix) radix_hist_scan_kernel(uint32_t *hist)
 {
@@ -371,6 +423,30 @@ __global__ void __launch_bounds__(256) iota_copy_kernel(int64_t n, const uint32_
     if (i < n) { sorted_hash[i] = hash[i]; perm[i] = (uint32_t)i; }
 }
 
+int launch_hash_hist(sph_ctx *c, int64_t n, const float *posm, uint32_t *hash)
+{
+    c->hist_for = nullptr;
+    const int P = c->n_passes;
+    if (n == 0 || P == 0) return launch_hash(c, n, posm, hash);
+    const int64_t tiles = (n + kSortTile - 1) / kSortTile;
+    const int64_t n_status = (int64_t)P * tiles * kRadix;
+    SPH_CUDA_TRY(c, cudaMemsetAsync(c->hist, 0, sizeof(uint32_t) * kMaxPasses * kRadix, c->stream));
+    int hb = (int)min((int64_t)c->num_sms * 8, (n + 1023) / 1024);
+    if (hb < 1) hb = 1;
+    const float4 *p4 = reinterpret_cast<const float4 *>(posm);
+    switch (P) {
+    case 1: hash_hist_kernel<1><<<hb, 256, 0, c->stream>>>(n, p4, hash, c->grid, c->hist, c->tile_status, n_status, c->tile_counter, kMaxPasses); break;
+    case 2: hash_hist_kernel<2><<<hb, 256, 0, c->stream>>>(n, p4, hash, c->grid, c->hist, c->tile_status, n_status, c->tile_counter, kMaxPasses); break;
+    case 3: hash_hist_kernel<3><<<hb, 256, 0, c->stream>>>(n, p4, hash, c->grid, c->hist, c->tile_status, n_status, c->tile_counter, kMaxPasses); break;
+    default: hash_hist_kernel<4><<<hb, 256, 0, c->stream>>>(n, p4, hash, c->grid, c->hist, c->tile_status, n_status, c->tile_counter, kMaxPasses); break;
+    }
+    SPH_CHECK_LAUNCH(c);
+    radix_hist_scan_kernel<<<P, kRadix, 0, c->stream>>>(c->hist);
+    SPH_CHECK_LAUNCH(c);
+    c->hist_for = hash;
+    return SPH_OK;
+}
+
 int launch_sort(sph_ctx *c, int64_t n, const uint32_t *hash, uint32_t *sorted_hash, uint32_t *perm)
 {
     if (n == 0) return SPH_OK;
@@ -381,6 +457,9 @@ int launch_sort(sph_ctx *c, int64_t n, const uint32_t *hash, uint32_t *sorted_ha
         return SPH_OK;
     }
     const int64_t tiles = (n + kSortTile - 1) / kSortTile;
+    const bool have_hist = c->hist_for == hash;   // sph_step: counted by the fused hash kernel
+    c->hist_for = nullptr;
+    if (!have_hist) {
     SPH_CUDA_TRY(c, cudaMemsetAsync(c->hist, 0, sizeof(uint32_t) * kMaxPasses * kRadix, c->stream));
     const int64_t n_status = (int64_t)P * tiles * kRadix;
     int hb = (int)min((int64_t)c->num_sms * 8, (n + 1023) / 1024);
@@ -394,6 +473,7 @@ int launch_sort(sph_ctx *c, int64_t n, const uint32_t *hash, uint32_t *sorted_ha
     SPH_CHECK_LAUNCH(c);
     radix_hist_scan_kernel<<<P, kRadix, 0, c->stream>>>(c->hist);
     SPH_CHECK_LAUNCH(c);
+    }
 
     {
         int rc = sort_smem_opt_in(c);
@@ -448,6 +528,7 @@ __global__ void segment_offsets_kernel(const uint32_t *__restrict__ hist_excl, i
 int launch_partition_keys(sph_ctx *c, int64_t m, int n_labels, uint32_t *offsets, uint32_t *dest, uint32_t **order)
 {
     uint32_t *key = c->alt_keys, *key_out = c->alt_vals, *val_out = c->s_comm_hash;  // scratch (stream-ordered)
+    c->hist_for = nullptr;   // the histogram scratch is reused below
     if (order) *order = val_out;
     if (m == 0) {
         SPH_CUDA_TRY(c, cudaMemsetAsync(offsets, 0, sizeof(uint32_t) * (n_labels + 1), c->stream));

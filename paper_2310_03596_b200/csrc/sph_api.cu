@@ -134,6 +134,7 @@ int sph_create(sph_ctx **out, const sph_params *p, int64_t max_n, void *cuda_str
     c->host_streams_ready = false;
     c->wait_before_reorder = nullptr;
     c->rec_fresh = false;
+    c->hist_for = nullptr;
     c->attr_sort = c->attr_interact = false;
     memset(&c->staging, 0, sizeof(c->staging));
 
@@ -332,7 +333,7 @@ static int step_impl(sph_ctx *c, int64_t n, float dt, const sph_state *state, ui
 
     int rc;
     StageTimer t(c);
-    if ((rc = launch_hash(c, n, state->posm, hash)) != SPH_OK) return rc;                  // step a
+    if ((rc = launch_hash_hist(c, n, state->posm, hash)) != SPH_OK) return rc;             // step a (+ the sort's histograms)
     t.mark();
     if ((rc = launch_sort(c, n, hash, sorted_hash, perm)) != SPH_OK) return rc;
     t.mark();
