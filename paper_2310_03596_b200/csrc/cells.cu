@@ -10,32 +10,36 @@ namespace sphb {
 constexpr int kCellItems = 8;  // sorted positions per thread (two 128-bit loads in flight)
 
 // boundary between sorted positions k-1 (hash hp) and k (hash hc): closes bucket hp, opens hc;
-// the empty buckets in between get start == end == k.  Returns the gap range for the caller.
-__device__ __forceinline__ void mark_boundary(int64_t k, int64_t n, int64_t hp, int64_t hc,
+// the empty buckets in between get start == end == k.  Everything is 32-bit: n < 2^30 and
+// n_cells < 2^32 - 1 (sph_create), the bucket before position 0 is passed as hp1 = hp + 1 = 0 and
+// the one behind position n - 1 as hc = n_cells.  A long gap is handed back to the caller.
+__device__ __forceinline__ void mark_boundary(uint32_t k, uint32_t n, uint32_t hp1, uint32_t hc,
                                               uint32_t *__restrict__ cs, uint32_t *__restrict__ ce,
-                                              int64_t &lo, int64_t &hi, uint32_t &fill)
+                                              uint32_t &lo, uint32_t &cnt, uint32_t &fill)
 {
-    if (hc == hp) return;
-    if (k < n) cs[hc] = (uint32_t)k;
-    if (k > 0) ce[hp] = (uint32_t)k;
-    const int64_t l = hp + 1, h = hc - 1;
-    if (h - l + 1 > 4) {        // at most one long gap is kept per thread; earlier ones are
-        if (hi >= lo)           // written inline (rare: two long gaps inside 8 positions)
-            for (int64_t c = lo; c <= hi; ++c) { cs[c] = fill; ce[c] = fill; }
-        lo = l; hi = h; fill = (uint32_t)k;
+    if (hc + 1u == hp1) return;                 // same bucket as the previous position
+    if (k < n) cs[hc] = k;
+    if (k > 0) ce[hp1 - 1u] = k;
+    const uint32_t gap = hc - hp1;              // empty buckets hp1 .. hc - 1
+    if (gap > 4u) {             // at most one long gap is kept per thread; earlier ones are
+        for (uint32_t c = 0; c < cnt; ++c) { cs[lo + c] = fill; ce[lo + c] = fill; }   // written inline (rare)
+        lo = hp1; cnt = gap; fill = k;
     } else {
-        for (int64_t c = l; c <= h; ++c) { cs[c] = (uint32_t)k; ce[c] = (uint32_t)k; }
+        for (uint32_t c = hp1; c < hc; ++c) { cs[c] = k; ce[c] = k; }
     }
 }
 
 __global__ void __launch_bounds__(256)
-cell_ranges_kernel(int64_t n, const uint32_t *__restrict__ sorted_hash, uint32_t *__restrict__ cs,
+cell_ranges_kernel(int64_t n64, const uint32_t *__restrict__ sorted_hash, uint32_t *__restrict__ cs,
                    uint32_t *__restrict__ ce, uint32_t n_cells)
 {
     // thread t owns the boundaries k = 8t .. 8t+7 (k == n closes the table)
-    const int64_t k0 = ((int64_t)blockIdx.x * blockDim.x + threadIdx.x) * kCellItems;
+    const uint32_t n = (uint32_t)n64;
+    // (k0 <= n + 8 * 256 < 2^31: no wrap; threads behind the last boundary mark nothing but stay
+    //  in the warp collectives)
+    const uint32_t k0 = (uint32_t)(((int64_t)blockIdx.x * blockDim.x + threadIdx.x) * kCellItems);
     const int lane = threadIdx.x & 31;
-    int64_t hcur[kCellItems];
+    uint32_t hcur[kCellItems];
     if (k0 + kCellItems <= n && (reinterpret_cast<uintptr_t>(sorted_hash) & 15) == 0) {
 #pragma unroll
         for (int q = 0; q < kCellItems / 4; ++q) {
@@ -45,27 +49,27 @@ cell_ranges_kernel(int64_t n, const uint32_t *__restrict__ sorted_hash, uint32_t
     } else {
 #pragma unroll
         for (int j = 0; j < kCellItems; ++j)
-            hcur[j] = (k0 + j < n) ? (int64_t)sorted_hash[k0 + j] : (int64_t)n_cells;
+            hcur[j] = (k0 + j < n) ? sorted_hash[k0 + j] : n_cells;
     }
-    // hash of position k0 - 1: the previous lane's last one, lane 0 reads it
-    int64_t hprev = __shfl_up_sync(0xffffffffu, hcur[kCellItems - 1], 1);
-    if (lane == 0) hprev = (k0 == 0) ? -1 : ((k0 - 1 < n) ? (int64_t)sorted_hash[k0 - 1] : (int64_t)n_cells);
-    int64_t lo = 0, hi = -1;  // long empty-bucket range [lo, hi] to fill with `fill`
+    // hash of position k0 - 1 (+ 1): the previous lane's last one, lane 0 reads it
+    uint32_t hp1 = __shfl_up_sync(0xffffffffu, hcur[kCellItems - 1], 1) + 1u;
+    if (lane == 0) hp1 = (k0 == 0) ? 0u : ((k0 - 1 < n) ? sorted_hash[k0 - 1] + 1u : n_cells + 1u);
+    uint32_t lo = 0, cnt = 0;   // long empty-bucket range [lo, lo + cnt) to fill with `fill`
     uint32_t fill = 0;
 #pragma unroll
     for (int j = 0; j < kCellItems; ++j) {
-        if (k0 + j <= n) mark_boundary(k0 + j, n, hprev, hcur[j], cs, ce, lo, hi, fill);
-        hprev = hcur[j];
+        if (k0 + j <= n) mark_boundary(k0 + j, n, hp1, hcur[j], cs, ce, lo, cnt, fill);
+        hp1 = hcur[j] + 1u;
     }
     // long gaps (config 3's clipped geometry has runs of thousands) are filled by the whole warp
-    uint32_t pending = __ballot_sync(0xffffffffu, hi >= lo);
+    uint32_t pending = __ballot_sync(0xffffffffu, cnt > 0);
     while (pending) {
         const int src = __ffs(pending) - 1;
         pending &= pending - 1;
-        const int64_t l = __shfl_sync(0xffffffffu, lo, src);
-        const int64_t h = __shfl_sync(0xffffffffu, hi, src);
+        const uint32_t l = __shfl_sync(0xffffffffu, lo, src);
+        const uint32_t m = __shfl_sync(0xffffffffu, cnt, src);
         const uint32_t f = __shfl_sync(0xffffffffu, fill, src);
-        for (int64_t c = l + lane; c <= h; c += 32) { cs[c] = f; ce[c] = f; }
+        for (uint32_t c = lane; c < m; c += 32) { cs[l + c] = f; ce[l + c] = f; }
     }
 }
 
