@@ -1,12 +1,15 @@
 // Stage 2a: hand-written onesweep LSD radix sort on (hash, id)  (reading S5).
 //
-// One histogram kernel reads the keys once and builds the digit histograms of every pass.
-// Each pass is then ONE kernel: a tile of 8192 keys is ranked with warp-level match/popc
+// One histogram kernel reads the keys once and builds the digit histograms of every pass (inside
+// sph_step the bucket-hash pass counts them instead, hash_hist_kernel below, and launch_sort skips
+// it).  Each pass is then ONE kernel: a tile of 6144 keys is ranked with warp-level match/popc
 // (stable), the tile's per-digit counts are chained to the previous tiles with decoupled
 // look-back (single 32-bit status word = 2 flag bits + 30-bit count, so no fence is needed), and
 // keys/values are staged through shared memory so each digit's run leaves as one contiguous
 // write.  Tiles take their index from an atomic ticket, which guarantees forward progress of the
-// look-back chain.  Values of the first pass are the implicit ids 0..n-1 (never read), and only
+// look-back chain; every tile also prefetches the keys / values of the tile one wave of resident
+// CTAs ahead into the L2 (the passes are bound by the bytes a tile has in flight, not by DRAM
+// bandwidth).  Values of the first pass are the implicit ids 0..n-1 (never read), and only
 // the live key bits ceil(log2(cells)) are sorted.  Stability + ascending ids on input give the
 // lexicographic (hash, id) order.
 #include "sph_internal.cuh"

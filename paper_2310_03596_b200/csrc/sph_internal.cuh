@@ -16,7 +16,7 @@ constexpr int kMaxPasses = 4;
 // onesweep tile geometry
 constexpr int kSortThreads = 384;
 constexpr int kSortItems = 16;
-constexpr int kSortTile = kSortThreads * kSortItems;  // 8192 keys per tile
+constexpr int kSortTile = kSortThreads * kSortItems;  // 6144 keys per tile
 
 // decoupled look-back status word: 2 flag bits + 30 value bits
 constexpr uint32_t kFlagAgg = 1u << 30;
