@@ -513,8 +513,17 @@ __global__ void __launch_bounds__(256)
 gather_label_kernel(int64_t m, const uint32_t *__restrict__ ids, const int32_t *__restrict__ label,
                     uint32_t *__restrict__ key)
 {
-    const int64_t k = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
-    if (k < m) key[k] = (uint32_t)__ldg(label + __ldcs(ids + k)) & (kRadix - 1);
+    // four independent id -> label chains per thread (a single dependent chain per thread left the
+    // kernel latency-bound: 294 us at 64 M entries with 15 % of the issue slots used)
+    const int64_t k0 = ((int64_t)blockIdx.x * blockDim.x) * 4 + threadIdx.x;
+    uint32_t id[4];
+#pragma unroll
+    for (int j = 0; j < 4; ++j) { const int64_t k = k0 + j * 256; id[j] = k < m ? __ldcs(ids + k) : 0u; }
+    uint32_t lb[4];
+#pragma unroll
+    for (int j = 0; j < 4; ++j) { const int64_t k = k0 + j * 256; lb[j] = k < m ? (uint32_t)__ldg(label + id[j]) : 0u; }
+#pragma unroll
+    for (int j = 0; j < 4; ++j) { const int64_t k = k0 + j * 256; if (k < m) key[k] = lb[j] & (kRadix - 1); }
 }
 
 __global__ void segment_offsets_kernel(const uint32_t *__restrict__ hist_excl, int n_labels, uint32_t m,
@@ -565,7 +574,7 @@ int launch_partition_by_label(sph_ctx *c, int64_t m, const uint32_t *ids, const 
     // then reads the list and the records in list order, which is sector-friendly, and writes
     // n_labels sequential streams -- the gather form re-read every sector once per label)
     if (m > 0) {
-        gather_label_kernel<<<div_up(m, 256), 256, 0, c->stream>>>(m, ids, label, c->alt_keys);
+        gather_label_kernel<<<div_up(m, 1024), 256, 0, c->stream>>>(m, ids, label, c->alt_keys);
         SPH_CHECK_LAUNCH(c);
     }
     return launch_partition_keys(c, m, n_labels, offsets, dest, nullptr);
