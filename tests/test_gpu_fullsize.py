@@ -23,7 +23,7 @@ from tests import parity
 
 pytestmark = pytest.mark.gpu
 
-N_SAMPLE = 3000
+N_SAMPLE = 20000
 
 
 @pytest.fixture(scope="module")
@@ -93,7 +93,19 @@ def _fullsize_case(sph, oracle, k, steps_before, expect_boundary):
 
     # ---- sampled float parity: sorted positions spread over the whole array + both ends -------
     rng = np.random.default_rng(4242 + k)
-    idx = np.unique(np.concatenate([rng.integers(0, n, N_SAMPLE), np.arange(64), np.arange(n - 64, n)]))
+    # ... + every particle of six complete interaction tiles (4 x 2 buckets of one layer: all work
+    # units of a tile, full and partial ones), two of them at the grid's edges
+    nx, ny, nz = (int(d) for d in w.dims)
+    tiles = [(0, 0, 0), ((nx - 1) // 4, (ny - 1) // 2, nz - 1)] + \
+            [(int(rng.integers(0, (nx + 3) // 4)), int(rng.integers(0, (ny + 1) // 2)), int(rng.integers(0, nz)))
+             for _ in range(4)]
+    tile_idx = []
+    for tx, ty, cz in tiles:
+        for cy in range(2 * ty, min(2 * ty + 2, ny)):
+            for cx in range(4 * tx, min(4 * tx + 4, nx)):
+                c = cx + nx * (cy + ny * cz)
+                tile_idx.append(np.arange(int(cs[c]), int(ce[c]), dtype=np.int64))
+    idx = np.unique(np.concatenate([rng.integers(0, n, N_SAMPLE), np.arange(64), np.arange(n - 64, n)] + tile_idx))
     sp, sv = posm[perm], velr[perm]
     ss = np.ascontiguousarray(sig[:, perm])
     rates = oracle.interact(sp, sv, ss, sh, w.dims, cs, ce, w.h, w.K, w.G, idx=idx)
@@ -129,7 +141,7 @@ def _fullsize_case(sph, oracle, k, steps_before, expect_boundary):
 
 def test_config1_full_size(sph, oracle):
     """configs[1], 1 M particles, the workload bench.py times by default: the oracle's integer
-    stages in full (bit-exact) and 3 000 sampled particles for the floats, at the LAST of the
+    stages in full (bit-exact) and 20 000 sampled particles + six complete tiles for the floats, at the LAST of the
     config's 10 steps (re-hash and re-sort every step)."""
     errs = _fullsize_case(sph, oracle, 1, steps_before=9, expect_boundary=(0.15, 0.27))
     assert max(errs.values()) <= parity.RATE_TOL
@@ -213,7 +225,7 @@ def test_balance_types_full_size(sph, oracle):
 
 def test_split_passes_config1_full_size(sph, oracle):
     """sph_interact_split (steps e / f) on configs[1] (1 M particles, 4 slabs) after
-    3 steps: each pass on 3 000 sampled sorted positions against orc_interact_split (normalised by
+    3 steps: each pass on 20 000 sampled sorted positions against orc_interact_split (normalised by
     the single pass's field maxima), pair counts add up, pass e + pass f = the single pass."""
     w = wl.config(1)
     ctx = sph.Context.for_workload(w)
