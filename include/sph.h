@@ -43,9 +43,11 @@ extern "C" {
 #define SPH_EINVAL   -1   /* null pointer, n < 0, n > max_n, bad params                         */
 #define SPH_ECUDA    -2   /* a CUDA runtime call or launch failed (see sph_last_cuda_error)     */
 #define SPH_ENOMEM   -3   /* scratch allocation failed                                           */
+#define SPH_ELIMIT   -4   /* size beyond the fixed capacity of sph_comm_hash_noalloc             */
 
 #define SPH_GARBAGE_HASH 0xFFFFFFFFu  /* PAPER.md:17 "some garbage collector hash" (reading S8) */
 #define SPH_MAX_OWNERS   32           /* paper's envelope is <= 16 GPUs           */
+#define SPH_NOALLOC_MAX_CELLS (1 << 22) /* buckets sph_comm_hash_noalloc's built-in scratch holds  */
 
 /* sph_params.flags */
 #define SPH_FLAG_INTERACT_DIRECT 1u   /* force the simple global-memory interaction kernel      */
@@ -260,6 +262,45 @@ int sph_step_varh(sph_ctx *ctx, int64_t n, float dt, const sph_state *state, con
  * steps). */
 int sph_step_host(sph_ctx *ctx, int64_t n, float dt, int32_t steps, const sph_state *host_state,
                   uint32_t *boundary_ids, uint32_t *boundary_count, unsigned long long *pair_count);
+
+/* Stage 3 for callers that cannot allocate device memory (step c).
+ *
+ * Every other entry point works on an sph_ctx, and sph_create obtains the ctx's scratch with
+ * cudaMalloc.  Some callers cannot do that: a solver that gave all device memory to its own pool at
+ * start-up, a plug-in whose host application forbids allocations (and the device-wide stall of a
+ * cudaFree) inside the time loop, a thread feeding a latency-critical stream that must stay clear of
+ * the allocator's locks.  For them this call needs NO ctx and calls no cudaMalloc, cudaFree or any
+ * allocating routine: its only scratch, one owner bitmask per bucket, is an array of
+ * SPH_NOALLOC_MAX_CELLS 32-bit words (16 MiB) built into the library image.  Every GPU that loads
+ * the library holds those 16 MiB until the process exits, used or not.
+ *
+ * Computes, for the same inputs, exactly sph_comm_hash's comm_hash and *boundary_count:
+ * comm_hash[k] = sorted_hash[k] if a particle with another owner lies in the 27-bucket stencil of
+ * k's bucket, else SPH_GARBAGE_HASH; *boundary_count = number of particles with comm_hash !=
+ * garbage.  The boundary list and the owner counts are not produced (they need tables this call has
+ * no room for); no cell_start / cell_end are needed.
+ * params: host; only dims and n_owners are read (dims > 0, n_owners in 1..SPH_MAX_OWNERS).
+ * In: sorted_hash, sorted_owner dev [n], n <= 2^30, sorted by hash, every hash < nx*ny*nz (a larger
+ * one gets the garbage hash and marks nothing, never a fault).  Out: comm_hash dev [n],
+ * boundary_count dev scalar -- caller-owned like everywhere else.  cuda_stream: a cudaStream_t
+ * (NULL = legacy default stream); the call only enqueues on it (two memsets, two kernels).
+ * The device is the CURRENT one; all pointers must belong to it.
+ *
+ * What the shared built-in array implies:
+ *  - Limit: nx*ny*nz > SPH_NOALLOC_MAX_CELLS is refused with SPH_ELIMIT before any CUDA call
+ *    (BASELINE.json's largest grid, 156^3 = 3.8 M buckets for 64 M particles, fits).
+ *  - It keeps the previous call's masks; each call first clears the words of its own grid.
+ *  - All calls on one GPU use the same array: calls whose work can overlap on the GPU (different
+ *    streams, or host threads that do not order their streams) race and give wrong flags.  Keep
+ *    them on one stream or order them with events.
+ *  - Set-up: the first call made while a given device is current looks up the array's address on
+ *    that device (cudaGetSymbolAddress, once per device, kept for the process).  Make that first
+ *    call before starting any stream capture.
+ * Errors: SPH_EINVAL (null pointer, n out of range, bad dims / n_owners, device ordinal >= 64),
+ * SPH_ELIMIT, SPH_ECUDA (the CUDA error is left pending: read it with cudaGetLastError). */
+int sph_comm_hash_noalloc(const sph_params *params, int64_t n, const uint32_t *sorted_hash,
+                          const int32_t *sorted_owner, uint32_t *comm_hash, uint32_t *boundary_count,
+                          void *cuda_stream);
 
 /* Per-stage device time of sph_step, measured with CUDA events recorded on the ctx's stream
  * (enabled by sph_enable_timing(ctx, 1); adds no host sync to sph_step itself -- sph_get_timing

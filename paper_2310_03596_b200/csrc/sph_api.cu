@@ -509,6 +509,7 @@ const char *sph_strerror(int code)
     case SPH_EINVAL: return "invalid argument";
     case SPH_ECUDA: return "CUDA error";
     case SPH_ENOMEM: return "out of device memory";
+    case SPH_ELIMIT: return "grid has more buckets than the built-in scratch of sph_comm_hash_noalloc holds (SPH_NOALLOC_MAX_CELLS)";
     default: return "unknown error";
     }
 }

@@ -21,7 +21,8 @@ import torch
 _HERE = os.path.dirname(os.path.abspath(__file__))
 LIB_PATH = os.path.join(_HERE, "libsph_b200.so")
 
-SPH_OK, SPH_EINVAL, SPH_ECUDA, SPH_ENOMEM = 0, -1, -2, -3
+SPH_OK, SPH_EINVAL, SPH_ECUDA, SPH_ENOMEM, SPH_ELIMIT = 0, -1, -2, -3, -4
+NOALLOC_MAX_CELLS = 1 << 22   # buckets the built-in scratch of sph_comm_hash_noalloc holds
 GARBAGE_HASH = 0xFFFFFFFF
 MAX_OWNERS = 32
 FLAG_INTERACT_DIRECT = 1
@@ -31,7 +32,7 @@ EXPORTS = (
     "sph_create", "sph_destroy", "sph_hash", "sph_sort", "sph_reorder", "sph_cell_ranges",
     "sph_comm_hash", "sph_interact", "sph_integrate", "sph_step", "sph_step_host", "sph_pack_boundary",
     "sph_interact_split", "sph_interact_varh", "sph_step_varh", "sph_interact_ef", "sph_balance", "sph_balance_types", "sph_enable_timing", "sph_get_timing", "sph_launch_count", "sph_strerror",
-    "sph_last_cuda_error",
+    "sph_last_cuda_error", "sph_comm_hash_noalloc",
 )
 
 
@@ -70,6 +71,7 @@ def load_library() -> C.CDLL:
     lib.sph_reorder.argtypes = [vp, i64, vp, sp, sp]
     lib.sph_cell_ranges.argtypes = [vp, i64, vp, vp, vp]
     lib.sph_comm_hash.argtypes = [vp, i64] + [vp] * 9
+    lib.sph_comm_hash_noalloc.argtypes = [C.POINTER(_Params), i64, vp, vp, vp, vp, vp]
     lib.sph_interact.argtypes = [vp, i64, sp, vp, vp, vp, vp, vp, C.POINTER(vp * 6), vp]
     lib.sph_interact_split.argtypes = [vp, i64, sp, vp, vp, vp, i32, vp, vp, C.POINTER(vp * 6), vp]
     lib.sph_interact_varh.argtypes = [vp, i64, sp, vp, vp, vp, vp, i32, vp, vp, C.POINTER(vp * 6), vp]
@@ -448,6 +450,40 @@ class Context:
                                          C.cast(C.byref(cnt), C.c_void_p),
                                          C.cast(C.byref(pc), C.c_void_p)), "sph_step_host")
         return int(cnt.value), int(pc.value)
+
+
+def sph_comm_hash_noalloc(dims, n_owners, sorted_hash: torch.Tensor, sorted_owner: torch.Tensor,
+                          comm_hash: torch.Tensor | None = None, boundary_count: torch.Tensor | None = None,
+                          stream=None):
+    """Communication hash for callers that may not allocate device memory (no Context, hence no
+    cudaMalloc: think of a solver whose own pool already owns the whole GPU, or a time loop in
+    which allocations are forbidden).  The C call uses a 16 MiB scratch array built into the
+    library instead; grids with more than NOALLOC_MAX_CELLS buckets raise (SPH_ELIMIT), calls that
+    overlap on one GPU race on that array, and the first call per device should come before any
+    stream capture.  Pass `comm_hash` [n] and `boundary_count` [1] (int32, on the tensors' device)
+    to keep this wrapper from allocating as well; they are created with torch otherwise.
+    Returns (comm_hash, boundary_count), valid once `stream` (default: torch's current) is synced."""
+    lib = load_library()
+    if not torch.cuda.is_available():
+        raise SphError("no CUDA device: the SPH path has no CPU fallback")
+    n = int(sorted_hash.shape[0])
+    dev = sorted_hash.device
+    p = _Params()
+    for a in range(3):
+        p.dims[a] = int(dims[a])
+    p.n_owners = int(n_owners)
+    if comm_hash is None:
+        comm_hash = torch.empty(n, dtype=torch.int32, device=dev)
+    if boundary_count is None:
+        boundary_count = torch.empty(1, dtype=torch.int32, device=dev)
+    with torch.cuda.device(dev):
+        st = stream if stream is not None else torch.cuda.current_stream(dev)
+        rc = lib.sph_comm_hash_noalloc(C.byref(p), n, sorted_hash.data_ptr(), sorted_owner.data_ptr(),
+                                       comm_hash.data_ptr(), boundary_count.data_ptr(),
+                                       C.c_void_p(st.cuda_stream))
+    if rc != SPH_OK:
+        raise SphError(f"sph_comm_hash_noalloc: {lib.sph_strerror(rc).decode()}")
+    return comm_hash, boundary_count
 
 
 # module-level aliases with the C names (ctx first, like the C-ABI)
