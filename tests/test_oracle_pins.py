@@ -184,9 +184,19 @@ def brute_comm_flags(posm, owner, origin, dims, h):
 
 
 @pytest.mark.parametrize("owners", [("plane_x", 5.0), ("random", 16), ("single",), ("slabs", 3),
-                                    ("slabs_mixed", 4, 0.02)])
+                                    ("slabs_mixed", 4, 0.02), ("rcb", 3), ("plane_y", 4.0),
+                                    ("plane_z", 5.0)])
 def test_comm_hash_and_boundary_bruteforce(owners):
-    w = W.lattice_block(11, 9, 10, 0.1, 77, owners=owners)
+    # rcb / plane_y / plane_z split the labels across y and z: a foreign particle is then found
+    # only through the -y / +y / -z / +z reach of the stencil ("the surrounding
+    # buckets": all 26), which x-splits and full mixing never exercise
+    if owners[0] in ("plane_y", "plane_z"):
+        w = W.lattice_block(11, 9, 10, 0.1, 77)
+        axis = 1 if owners[0] == "plane_y" else 2
+        w.owner = np.where(w.posm[:, axis] < np.float32(owners[1]), 0, 1).astype(np.int32)
+        w.n_owners = 2
+    else:
+        w = W.lattice_block(11, 9, 10, 0.1, 77, owners=owners)
     r, sp, sv, ss, so = sorted_view(w)
     flags = brute_comm_flags(w.posm, w.owner, w.origin, w.dims, w.h)       # id order
     exp_comm = np.where(flags[r.perm], r.sorted_hash, np.uint32(orc.GARBAGE))
@@ -209,6 +219,30 @@ def test_comm_hash_and_boundary_bruteforce(owners):
         assert r.boundary_ids.size == 0                   # I10 / S12
     if owners[0] == "random":
         assert r.boundary_ids.size == w.n                 # PAPER.md:30 full mixing
+
+
+def test_one_foreign_particle_flags_exactly_its_27_buckets():
+    """one particle of another GPU in an interior bucket makes boundary particles of
+    exactly the particles in that bucket and its 26 surrounding ones -- every direction counts."""
+    w = W.lattice_block(14, 13, 12, 0.1, 78)
+    c = bucket_coords_f32(w.posm, w.origin, w.dims, w.h)
+    inner = np.nonzero((c == np.array([2, 2, 2])).all(1))[0]       # bucket (2,2,2): not at the grid's edge
+    assert inner.size > 0 and (np.array(w.dims) >= 5).all()
+    w.owner = np.zeros(w.n, np.int32)
+    w.owner[inner[0]] = 1
+    w.n_owners = 2
+    r, *_ = sorted_view(w)
+    flagged = np.zeros(w.n, bool)
+    flagged[r.perm[r.comm_hash != orc.GARBAGE]] = True
+    near = (np.abs(c - c[inner[0]]) <= 1).all(1)
+    # the foreign particle's own bucket holds owner-0 particles too, so it is flagged as well
+    assert (w.owner[inner] == 0).any()
+    assert np.array_equal(flagged, near)
+    # all 27 buckets are occupied and flagged, none beyond
+    fb = np.unique(c[flagged], axis=0)
+    assert fb.shape[0] == 27 and (fb.min(0) == 1).all() and (fb.max(0) == 3).all()
+    assert np.array_equal(np.sort(r.boundary_ids), np.nonzero(near)[0].astype(np.uint32))
+    assert np.array_equal(flagged, brute_comm_flags(w.posm, w.owner, w.origin, w.dims, w.h))
 
 
 def test_boundary_slabs_lie_on_surfaces():
