@@ -685,6 +685,28 @@ def test_balance_hand_worked_example_golden():
     np.testing.assert_array_equal(own, [int(r[4]) for r in rows])
 
 
+def test_balance_three_owner_pair_order_golden():
+    """Reading B1 ("repeated for each GPU pair"): pairs (0,1), (0,2), (1,2) in this
+    order, each with the labels and centres of gravity the previous pair left.  Worked by hand in
+    tests/golden/balancing_three_owner_example.txt; every other pair order and Cgs frozen at the
+    start of the sweep give other hashes / labels / swap counts.  The typed sweep with one type and
+    alpha = 0 is the same computation (Cg' = Cg_type) and must give the same rows."""
+    rows = [l.split() for l in open(os.path.join(GOLDEN, "balancing_three_owner_example.txt"))
+            if l.strip() and not l.startswith("#")]
+    posm = np.zeros((len(rows), 4), np.float32)
+    posm[:, 0] = [float(r[1]) for r in rows]; posm[:, 3] = 1
+    own0 = np.array([int(r[2]) for r in rows], np.int32)
+    want_hash, want_own = [int(r[3]) for r in rows], [int(r[4]) for r in rows]
+    own, k, bh = orc.balance(posm, own0, 3)
+    assert k == 3
+    np.testing.assert_array_equal(bh, want_hash)
+    np.testing.assert_array_equal(own, want_own)
+    own_t, k_t, bh_t = orc.balance_types(posm, own0, np.zeros(len(rows), np.int32), 3, 1, alpha=0.0)
+    assert k_t == 3
+    np.testing.assert_array_equal(bh_t, want_hash)
+    np.testing.assert_array_equal(own_t, want_own)
+
+
 def test_balance_keeps_counts_slabs_are_a_fixed_point_single_owner_noop():
     """'The computational workload will stay balanced for all the swapping operations'
     (PAPER.md:30): every swap exchanges one particle each way; a slab decomposition has no
