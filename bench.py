@@ -266,18 +266,22 @@ def run_ours(args, rank, world, local_rank):
         torch.cuda.synchronize(dev)
         m_b = int(sph.as_u32(o2.boundary_count)[0])
         pk_ms = []
+        pk_out = (torch.empty(w.n_owners + 1, dtype=torch.int32, device=dev),
+                  torch.empty(max(m_b, 1), dtype=torch.int32, device=dev), sph.State.empty(max(m_b, 1), dev))
         for _ in range(5):
             flush.zero_()
             a_, b_ = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
             a_.record()
-            ctx.sph_pack_boundary(state, o2.boundary_ids, m_b)
+            ctx.sph_pack_boundary(state, o2.boundary_ids, m_b, out=pk_out)
             b_.record()
             torch.cuda.synchronize(dev)
             pk_ms.append(a_.elapsed_time(b_))
         pk = float(np.median(pk_ms[1:]))
+        pk_gbs = 156.0 * m_b / (pk * 1e-3) / 1e9 if pk > 0 else 0.0
         pack = {"ms": round(pk, 4), "boundary_particles": m_b, "bytes_per_boundary_particle": 156,
-                "note": "includes the allocation of the output tensors by the binding"}
-        del o2, bids_dev, bcnt
+                "gbs": round(pk_gbs, 1), "hbm_frac": round(pk_gbs / load_peaks()["hbm_gbs"], 3),
+                "note": "outputs pre-allocated (no allocation inside the timed interval)"}
+        del o2, bids_dev, bcnt, pk_out
 
     # ---- NEXT-3 (not part of the step metric): steps e / f as separate interaction passes ----
     split = None
@@ -326,11 +330,22 @@ def run_ours(args, rank, world, local_rank):
             b_.record()
             torch.cuda.synchronize(dev)
             ms_b.append(a_.elapsed_time(b_))
+            del _bh
             swaps.append(int(sw_.cpu()[0]))
             ctx.sph_step(st_b.clone(), w.dt, o_b)
             torch.cuda.synchronize(dev)
             frac.append(int(sph.as_u32(o_b.boundary_count)[0]) / n)
-        bal = {"sweep_ms": [round(x, 3) for x in ms_b], "swapped_pairs": swaps,
+        # the same sweep with the optional bal_hash output stored (the parity tests' form), on a copy
+        own_h = st_b.owner.clone()
+        a_, b_ = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        a_.record()
+        _bh, _sw = ctx.sph_balance(st_b.posm, own_h, want_hash=True)
+        b_.record()
+        torch.cuda.synchronize(dev)
+        ms_with_hash = a_.elapsed_time(b_)
+        del own_h, _bh, _sw
+        bal = {"sweep_ms": [round(x, 3) for x in ms_b], "sweep_ms_note": "bal_hash not stored (optional output NULL)",
+               "sweep_ms_hashes_stored": round(ms_with_hash, 3), "swapped_pairs": swaps,
                "boundary_fraction": [round(x, 4) for x in frac], "owner_pairs": w.n_owners * (w.n_owners - 1) // 2}
         del st_b, o_b
 
@@ -360,11 +375,16 @@ def run_ours(args, rank, world, local_rank):
     fp32_peak = fp32_peak_tflops(props.multi_processor_count, peaks["sm_max_mhz"])
     achieved_tf = flops / t_int / 1e12
     stages = {}
+    n_sort_passes = (max(1, int(np.ceil(np.log2(max(2, w.n_cells))))) + 7) // 8
     for k_, v in stage_ms.items():
         e = {"ms": round(v, 4)}
         b = BYTES_PER_PARTICLE.get(k_)
         if k_ == "sort":
-            b = 4.0 + 16.0 * ((max(1, int(np.ceil(np.log2(max(2, w.n_cells))))) + 7) // 8)
+            # inside sph_step the digit histograms are counted by the fused hash kernel, so this
+            # stage is the onesweep passes alone: 16 B per particle and pass (keys + values in and
+            # out).  The 4 B histogram read of SURVEY.md's 52 B/p belongs to stand-alone sph_sort.
+            b = 16.0 * n_sort_passes
+            e["note"] = f"{n_sort_passes} onesweep passes only (16 B/p each); histograms are in the hash stage"
         if k_ == "cell_ranges":
             b = 4.0 + 8.0 * w.n_cells / n
         if k_ == "comm_hash":
@@ -380,6 +400,15 @@ def run_ours(args, rank, world, local_rank):
             e["gbs"] = round(b * n / (v * 1e-3) / 1e9, 1)
             e["hbm_frac"] = round(e["gbs"] / peaks["hbm_gbs"], 3)
         stages[k_] = e
+    # hash + sort as ONE fused stage on SURVEY.md 8(a)'s bytes (20 B/p hash + 4 B/p histogram read
+    # + 16 B/p per pass): the fusion moved the histogram's bytes AND time into the hash kernel, so
+    # only the sum can be compared with the survey's per-stage table
+    hs_ms = stage_ms["hash"] + stage_ms["sort"]
+    if hs_ms > 0:
+        hs_b = 20.0 + 4.0 + 16.0 * n_sort_passes
+        hs_gbs = hs_b * n / (hs_ms * 1e-3) / 1e9
+        stages["hash_plus_sort"] = {"ms": round(hs_ms, 4), "bytes_per_particle": hs_b, "gbs": round(hs_gbs, 1),
+                                    "hbm_frac": round(hs_gbs / peaks["hbm_gbs"], 3)}
     line = {
         "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": K, "warmup": W,
         "ms_per_step": ms_per_step, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,

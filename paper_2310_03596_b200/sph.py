@@ -426,13 +426,19 @@ class Context:
                   "sph_balance_types")
         return bh[:n], sw
 
-    def sph_pack_boundary(self, state: State, boundary_ids: torch.Tensor, m: int):
+    def sph_pack_boundary(self, state: State, boundary_ids: torch.Tensor, m: int, out=None):
         """Per-owner send buffers (NEXT-1): returns (owner_offsets [n_owners + 1], packed_ids [m],
-        packed State of length m).  m is the host value of boundary_count."""
+        packed State of length m).  m is the host value of boundary_count.  out = (offsets, ids,
+        State) of capacity >= m re-uses caller tensors (the State's length is the sig plane stride)."""
         m = int(m)
-        offs = self._i32(self.n_owners + 1)
-        ids = self._i32(max(m, 1))
-        packed = State.empty(max(m, 1), self.device)
+        if out is not None:
+            offs, ids, packed = out
+            if offs.numel() < self.n_owners + 1 or ids.numel() < m or packed.n < m:
+                raise SphError("sph_pack_boundary: out tensors too small")
+        else:
+            offs = self._i32(self.n_owners + 1)
+            ids = self._i32(max(m, 1))
+            packed = State.empty(max(m, 1), self.device)
         a, b = state._c(), packed._c()
         self._chk(self.lib.sph_pack_boundary(self.handle, state.n, m, C.byref(a), boundary_ids.data_ptr(),
                                              offs.data_ptr(), ids.data_ptr(), C.byref(b)), "sph_pack_boundary")

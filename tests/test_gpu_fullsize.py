@@ -73,26 +73,12 @@ def _check_unique_integer_products(oracle, w, posm, owner, out, n):
     return sh, perm, cs, ce, m
 
 
-def _fullsize_case(sph, oracle, k, steps_before, expect_boundary):
-    w = wl.config(k)
+def _check_sampled_floats(sph, oracle, ctx, w, k, step, state, out, before, ints, last):
+    """Float rates and the integrated state on sampled sorted positions + whole tiles (reading S20)."""
+    posm, velr, sig, owner = before
+    sh, perm, cs, ce, m = ints
     n = w.n
-    ctx = sph.Context.for_workload(w)
-    state = sph.State.from_numpy(w.posm, w.velr, w.sig, w.owner)
-    for _ in range(steps_before):                      # the bench's launch configuration
-        ctx.sph_step(state, w.dt)
-    torch.cuda.synchronize()
-    posm, velr = state.posm.cpu().numpy(), state.velr.cpu().numpy()
-    sig, owner = state.sig.cpu().numpy(), state.owner.cpu().numpy()
-    out = ctx.alloc_outputs(n)
-    ctx.sph_step(state, w.dt, out)
-    torch.cuda.synchronize()
-
-    sh, perm, cs, ce, m = _check_unique_integer_products(oracle, w, posm, owner, out, n)
-    lo, hi = expect_boundary
-    assert lo * n <= m <= hi * n, (m, n)
-
-    # ---- sampled float parity: sorted positions spread over the whole array + both ends -------
-    rng = np.random.default_rng(4242 + k)
+    rng = np.random.default_rng(4242 + k + 1000 * step)
     # ... + every particle of six complete interaction tiles (4 x 2 buckets of one layer: all work
     # units of a tile, full and partial ones), two of them at the grid's edges
     nx, ny, nz = (int(d) for d in w.dims)
@@ -110,7 +96,10 @@ def _fullsize_case(sph, oracle, k, steps_before, expect_boundary):
     ss = np.ascontiguousarray(sig[:, perm])
     rates = oracle.interact(sp, sv, ss, sh, w.dims, cs, ce, w.h, w.K, w.G, idx=idx)
     errs = parity.compare_rates(out, rates, idx=idx)
+    assert max(errs.values()) <= parity.RATE_TOL, (step, errs)
     assert max(np.max(np.abs(rates.drho)), np.max(np.abs(rates.dsig))) > 0, "sample exercises no float path"
+    if step > 1:
+        assert np.max(np.abs(rates.acc)) > 0, "momentum loop not exercised"    # sigma != 0 from step 2 on
     # integrated state of the sampled particles (O9), compared in id order
     po, vo, so = oracle.integrate(w.dt, sp[idx], sv[idx], np.ascontiguousarray(ss[:, idx]),
                                   rates.drho, rates.acc, rates.dsig)
@@ -122,7 +111,10 @@ def _fullsize_case(sph, oracle, k, steps_before, expect_boundary):
     for name, g, r in (("pos", g_pos[:, :3], po[:, :3]), ("vel", g_vel[:, :3], vo[:, :3]),
                        ("rho", g_vel[:, 3], vo[:, 3]), ("sig", g_sig, so)):
         e = parity.field_err(g, r)
-        assert e <= parity.STATE_TOL, (name, e)
+        assert e <= parity.STATE_TOL, (step, name, e)
+    del sp, sv, ss
+    if not last:
+        return errs
     # NEXT-1: per-owner send buffers of this step's boundary list, from the integrated state
     offs, pids, packed = ctx.sph_pack_boundary(state, out.boundary_ids, m)
     torch.cuda.synchronize()
@@ -132,38 +124,78 @@ def _fullsize_case(sph, oracle, k, steps_before, expect_boundary):
     np.testing.assert_array_equal(parity.u32(pids), ref.ids)
     np.testing.assert_array_equal(packed.posm.cpu().numpy(), ref.posm)
     np.testing.assert_array_equal(packed.sig.cpu().numpy(), ref.sig)
-    del packed, ref
-    # untouched particles elsewhere keep mass and owner
+    return errs
+
+
+def _fullsize_case(sph, oracle, k, int_steps, float_steps, expect_boundary):
+    """Reading S20 at full size: ALL of the config's steps run on the GPU in the bench's launch
+    configuration (sph_step on the id-ordered state, re-hash / re-sort / comm hash / compaction
+    every step); on the steps in `int_steps` every integer product is compared with the oracle, on
+    those in `float_steps` (a subset: first, middle, last) also the float rates and the integrated
+    state.  The oracle is re-seeded from the GPU's state before every compared step (lock-step)."""
+    w = wl.config(k)
+    n = w.n
+    assert set(float_steps) <= set(int_steps) and max(int_steps) == w.steps
+    ctx = sph.Context.for_workload(w)
+    state = sph.State.from_numpy(w.posm, w.velr, w.sig, w.owner)
+    out = ctx.alloc_outputs(n)
+    owner = w.owner
+    errs = {}
+    for step in range(1, w.steps + 1):
+        if step not in int_steps:
+            ctx.sph_step(state, w.dt)
+            continue
+        torch.cuda.synchronize()
+        posm = state.posm.cpu().numpy()
+        floats = step in float_steps
+        before = (posm, state.velr.cpu().numpy(), state.sig.cpu().numpy(), owner) if floats else None
+        ctx.sph_step(state, w.dt, out)
+        torch.cuda.synchronize()
+        ints = _check_unique_integer_products(oracle, w, posm, owner, out, n)
+        lo, hi = expect_boundary
+        assert lo * n <= ints[4] <= hi * n, (step, ints[4], n)
+        if floats:
+            errs = _check_sampled_floats(sph, oracle, ctx, w, k, step, state, out, before, ints,
+                                         last=step == w.steps)
+        del before, ints, posm
+    # mass and owner labels are carried through every step untouched
     np.testing.assert_array_equal(state.owner.cpu().numpy(), owner)
+    np.testing.assert_array_equal(state.posm[:, 3].cpu().numpy(), w.posm[:, 3])
     ctx.close()
     return errs
 
 
 def test_config1_full_size(sph, oracle):
-    """configs[1], 1 M particles, the workload bench.py times by default: the oracle's integer
-    stages in full (bit-exact) and 20 000 sampled particles + six complete tiles for the floats, at the LAST of the
-    config's 10 steps (re-hash and re-sort every step)."""
-    errs = _fullsize_case(sph, oracle, 1, steps_before=9, expect_boundary=(0.15, 0.27))
+    """configs[1], 1 M particles, all 10 steps: the oracle's integer stages in full (bit-exact) on
+    EVERY step, 20 000 sampled particles + six complete tiles for the floats on steps 1, 5, 10."""
+    errs = _fullsize_case(sph, oracle, 1, int_steps=range(1, 11), float_steps=(1, 5, 10),
+                          expect_boundary=(0.15, 0.27))
     assert max(errs.values()) <= parity.RATE_TOL
 
 
 def test_config2_full_size(sph, oracle):
-    """configs[2], 8 M particles, volumetric exchange region (everything is a boundary particle);
-    checked at the last of its 10 steps."""
-    _fullsize_case(sph, oracle, 2, steps_before=9, expect_boundary=(0.999, 1.0))
+    """configs[2], 8 M particles, volumetric exchange region (everything is a boundary particle):
+    integers on every one of its 10 steps, floats on steps 1, 5, 10."""
+    _fullsize_case(sph, oracle, 2, int_steps=range(1, 11), float_steps=(1, 5, 10),
+                   expect_boundary=(0.999, 1.0))
 
 
 @pytest.mark.skipif(os.environ.get("SPH_SKIP_64M") == "1", reason="SPH_SKIP_64M=1")
 def test_config4_full_size(sph, oracle):
-    """configs[4], 64 M particles (the maximum size): 22-bit keys, 7 813 onesweep tiles."""
-    _fullsize_case(sph, oracle, 4, steps_before=1, expect_boundary=(0.999, 1.0))
+    """configs[4], 64 M particles (the maximum size; 22-bit keys, 7 813 onesweep tiles): all 20
+    steps with a full re-hash, re-sort, comm hash and compaction each; integers and floats compared
+    on the first, the middle and the last step (reading S20 for configs[3], [4])."""
+    _fullsize_case(sph, oracle, 4, int_steps=(1, 10, 20), float_steps=(1, 10, 20),
+                   expect_boundary=(0.999, 1.0))
 
 
 @pytest.mark.skipif(os.environ.get("SPH_SKIP_22M") == "1", reason="SPH_SKIP_22M=1")
 def test_config3_full_size(sph, oracle):
     """configs[3], the irregular geometry as stated (22.0 M particles: plate + 8 cylinders, long
-    runs of empty buckets, 16 owners by recursive coordinate bisection)."""
-    _fullsize_case(sph, oracle, 3, steps_before=1, expect_boundary=(0.05, 0.35))
+    runs of empty buckets, 16 owners by recursive coordinate bisection): all 10 steps, compared on
+    steps 1, 5, 10."""
+    _fullsize_case(sph, oracle, 3, int_steps=(1, 5, 10), float_steps=(1, 5, 10),
+                   expect_boundary=(0.05, 0.35))
 
 
 # ------------------------------------------------------------------ NEXT items at full size

@@ -582,3 +582,69 @@ def test_long_run_then_lockstep(sph, oracle):
     parity.compare_rates(out, ref.rates)
     parity.compare_state(state, ref)
     ctx.close()
+
+
+def test_balancing_cadence_inside_a_run(sph, oracle):
+    """PAPER.md:32 "activate the balancing algorithm every 20 integration loops": 20 sph_steps, one
+    sph_balance sweep on the positions the run has reached (bit-exact labels against the oracle),
+    then the step AFTER the labels changed in lock-step against the oracle -- the new labels must
+    reach the communication hash, the boundary list and the owner counts; twice in a row."""
+    w = wl.config(2, side=37)
+    g = w.n_owners
+    ctx = sph.Context.for_workload(w)
+    state = sph.State.from_numpy(w.posm, w.velr, w.sig, w.owner)
+    out = ctx.alloc_outputs(w.n)
+    count0 = np.bincount(w.owner, minlength=g)
+    boundary = []
+    for cycle in range(2):
+        for _ in range(20):
+            ctx.sph_step(state, w.dt)
+        torch.cuda.synchronize()
+        posm = state.posm.cpu().numpy()
+        own_before = state.owner.cpu().numpy()
+        own_ref, k, bh_ref = oracle.balance(posm, own_before, g)
+        bh, sw = ctx.sph_balance(state.posm, state.owner)
+        torch.cuda.synchronize()
+        assert int(sw.cpu()[0]) == k and k > 0, (cycle, k)
+        np.testing.assert_array_equal(bh.cpu().numpy(), bh_ref)
+        np.testing.assert_array_equal(state.owner.cpu().numpy(), own_ref)
+        np.testing.assert_array_equal(np.bincount(own_ref, minlength=g), count0)
+        # the step after the sweep, from the GPU's state with the NEW labels
+        velr, sig = state.velr.cpu().numpy(), state.sig.cpu().numpy()
+        ref = oracle.step(posm, velr, sig, own_ref, w.origin, w.dims, w.h, w.K, w.G, g, w.dt)
+        stale = oracle.step(posm, velr, sig, own_before, w.origin, w.dims, w.h, w.K, w.G, g, w.dt, floats=False)
+        assert not np.array_equal(ref.comm_hash, stale.comm_hash) or \
+            not np.array_equal(ref.owner_counts, stale.owner_counts)   # the sweep changed stage 3's product
+        ctx.sph_step(state, w.dt, out)
+        torch.cuda.synchronize()
+        parity.compare_integers(out, ref, w.n)
+        parity.compare_rates(out, ref.rates)
+        parity.compare_state(state, ref)
+        np.testing.assert_array_equal(state.owner.cpu().numpy(), own_ref)
+        boundary.append(int(ref.boundary_ids.shape[0]))
+    ctx.close()
+
+
+def test_balance_three_owner_golden_example_on_the_gpu(sph):
+    """The hand-worked three-owner sweep of tests/golden/balancing_three_owner_example.txt (pair
+    order (0,1), (0,2), (1,2), Cgs recomputed after every pair -- reading B1) through
+    sph_balance and sph_balance_types (one type, alpha = 0): compared with the file, not the oracle."""
+    import os
+    path = os.path.join(os.path.dirname(__file__), "golden", "balancing_three_owner_example.txt")
+    rows = [l.split() for l in open(path) if l.strip() and not l.startswith("#")]
+    posm = np.zeros((len(rows), 4), np.float32)
+    posm[:, 0] = [float(r[1]) for r in rows]; posm[:, 3] = 1
+    own0 = np.array([int(r[2]) for r in rows], np.int32)
+    ctx = sph.Context(origin=(-1.0, -1.0, -1.0), dims=(8, 2, 2), h=1.0, n_owners=3, max_n=len(rows))
+    p = torch.from_numpy(posm).cuda()
+    for typed in (False, True):
+        own = torch.from_numpy(own0.copy()).cuda()
+        if typed:
+            bh, sw = ctx.sph_balance_types(p, own, torch.zeros(len(rows), dtype=torch.int32, device="cuda"), 1, 0.0)
+        else:
+            bh, sw = ctx.sph_balance(p, own)
+        torch.cuda.synchronize()
+        assert int(sw.cpu()[0]) == 3
+        np.testing.assert_array_equal(bh.cpu().numpy(), [int(r[3]) for r in rows])
+        np.testing.assert_array_equal(own.cpu().numpy(), [int(r[4]) for r in rows])
+    ctx.close()
