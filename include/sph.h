@@ -56,7 +56,7 @@ typedef struct sph_ctx sph_ctx;      /* opaque */
 
 typedef struct {
     float    origin[3];  /* lower corner of the bucket grid (reading S3)                        */
-    int32_t  dims[3];    /* nx, ny, nz buckets; nx*ny*nz < 2^32 - 1                              */
+    int32_t  dims[3];    /* nx, ny, nz buckets; each 1 .. 2^24, nx*ny*nz < 2^32 - 1              */
     float    h;          /* smoothing length (the MAXIMUM one with sph_*_varh); bucket edge = 2h   */
     float    K, G;       /* bulk / shear modulus of the linear-elastic law (BASELINE.json cfgs)  */
     int32_t  n_owners;   /* 1 .. SPH_MAX_OWNERS                                                  */
@@ -72,7 +72,7 @@ typedef struct {          /* SoA particle state; every pointer dev, length n    
 
 /* Create a context: validates params, allocates scratch for max_n particles on the current
  * device.  cuda_stream is a cudaStream_t (borrowed; NULL = legacy default stream).
- * Errors: SPH_EINVAL (null, max_n < 0 or >= 2^30, dims <= 0 or product >= 2^32-1, h <= 0 or not
+ * Errors: SPH_EINVAL (null, max_n < 0 or >= 2^30, a dim <= 0 or > 2^24, product >= 2^32-1, h <= 0 or not
  * finite, n_owners outside 1..32), SPH_ENOMEM, SPH_ECUDA. */
 int sph_create(sph_ctx **ctx, const sph_params *params, int64_t max_n, void *cuda_stream);
 int sph_destroy(sph_ctx *ctx);

@@ -629,7 +629,9 @@ interact_tiled_kernel(Packed rec, InteractIn in, const uint32_t *__restrict__ cs
                     si[3] = rc.y * rho2; si[4] = rd.x * rho2; si[5] = rd.y * rho2;
                     float4 pos_i = make_float4(0.f, 0.f, 0.f, 0.f);
                     if (out.perm) pos_i = __ldg(in.posm + i);
-                    finish_particle(Rr, si, rho, k, out, (int64_t)i, pos_i, rb.x, rb.y, rb.z);
+                    // same routing as the in-loop epilogue: kPassBoth parks step e in slot 0, step f in slot 1
+                    const InteractOut &oo = (kMode == kPassBoth && lane >= 4) ? out_f : out;
+                    finish_particle(Rr, si, rho, k, oo, (int64_t)i, pos_i, rb.x, rb.y, rb.z);
                 }
             }
         }

@@ -88,8 +88,14 @@ struct StageTimer {
     int idx = 0, slot = 0;
     explicit StageTimer(sph_ctx *ctx) : c(ctx)
     {
-        if (c->timing.on) slot = (int)(c->timing.count++ % kTimingSlots);
+        // the slot is claimed here but only counted by commit(), after the last mark of a step
+        // that enqueued completely: a step that fails midway leaves no half-recorded slot behind
+        if (c->timing.on) slot = (int)(c->timing.count % kTimingSlots);
         mark();
+    }
+    void commit()
+    {
+        if (c->timing.on) c->timing.count++;
     }
     void mark()
     {
@@ -117,7 +123,9 @@ int sph_create(sph_ctx **out, const sph_params *p, int64_t max_n, void *cuda_str
     if (p->n_owners < 1 || p->n_owners > SPH_MAX_OWNERS) return SPH_EINVAL;
     uint64_t cells = 1;
     for (int a = 0; a < 3; ++a) {
-        if (p->dims[a] <= 0) return SPH_EINVAL;
+        // above 2^24 a bucket coordinate is no longer exact in fp32 (clamping to (float)(n - 1)
+        // and clamping the converted integer to n - 1 would differ): such grids are refused
+        if (p->dims[a] <= 0 || p->dims[a] > (1 << 24)) return SPH_EINVAL;
         cells *= (uint64_t)p->dims[a];
         if (cells >= 0xFFFFFFFFull) return SPH_EINVAL;
     }
@@ -132,6 +140,7 @@ int sph_create(sph_ctx **out, const sph_params *p, int64_t max_n, void *cuda_str
     c->last_err = cudaSuccess;
     c->staging_ready = false;
     c->host_streams_ready = false;
+    c->h_count = nullptr;
     c->wait_before_reorder = nullptr;
     c->rec_fresh = false;
     c->hist_for = nullptr;
@@ -185,6 +194,7 @@ int sph_destroy(sph_ctx *c)
         cudaEventDestroy(c->ev_posm);
         cudaEventDestroy(c->ev_rest);
         cudaStreamDestroy(c->copy_stream);
+        cudaFreeHost(c->h_count);
     }
     cudaFree(c->arena);
     delete c;
@@ -357,6 +367,7 @@ static int step_impl(sph_ctx *c, int64_t n, float dt, const sph_state *state, ui
         return rc;
     t.mark();
     t.mark();
+    t.commit();
     return SPH_OK;
 }
 
@@ -396,10 +407,9 @@ int sph_interact_varh(sph_ctx *c, int64_t n, const sph_state *sorted, const floa
                            which, sorted_h);
 }
 
-int sph_step_host(sph_ctx *c, int64_t n, float dt, int32_t steps, const sph_state *hs,
-                  uint32_t *boundary_ids, uint32_t *boundary_count, unsigned long long *pair_count)
+static int step_host_impl(sph_ctx *c, int64_t n, float dt, int32_t steps, const sph_state *hs,
+                          uint32_t *boundary_ids, uint32_t *boundary_count, unsigned long long *pair_count)
 {
-    if (!n_ok(c, n) || !state_ok(hs) || steps < 0) return SPH_EINVAL;
     if (!c->staging_ready) {
         const size_t m = (size_t)(c->max_n > 0 ? c->max_n : 1);
         char *base = nullptr;
@@ -420,6 +430,9 @@ int sph_step_host(sph_ctx *c, int64_t n, float dt, int32_t steps, const sph_stat
         SPH_CUDA_TRY(c, cudaStreamCreateWithFlags(&c->copy_stream, cudaStreamNonBlocking));
         SPH_CUDA_TRY(c, cudaEventCreateWithFlags(&c->ev_posm, cudaEventDisableTiming));
         SPH_CUDA_TRY(c, cudaEventCreateWithFlags(&c->ev_rest, cudaEventDisableTiming));
+        // pinned landing word for the boundary count (an async D2H into pageable stack memory
+        // would only be safe because of the synchronisation that follows it)
+        SPH_CUDA_TRY(c, cudaHostAlloc(reinterpret_cast<void **>(&c->h_count), sizeof(uint32_t), cudaHostAllocDefault));
         c->host_streams_ready = true;
     }
     // posm first, on the ctx's stream: hash, sort and nothing else of the step can start on it.
@@ -439,7 +452,7 @@ int sph_step_host(sph_ctx *c, int64_t n, float dt, int32_t steps, const sph_stat
     for (int32_t it = 0; it < steps; ++it) {
         int rc = step_impl(c, n, dt, &d, nullptr, nullptr, nullptr, nullptr, nullptr, nullptr, nullptr,
                            nullptr, nullptr, nullptr, nullptr, nullptr, c->s_pair_count, false);
-        if (rc != SPH_OK) { c->wait_before_reorder = nullptr; cudaStreamSynchronize(s2); return rc; }
+        if (rc != SPH_OK) return rc;
     }
     if (c->wait_before_reorder) {   // steps == 0: nothing has waited for the second upload yet
         SPH_CUDA_TRY(c, cudaStreamWaitEvent(s, c->wait_before_reorder, 0));
@@ -451,9 +464,10 @@ int sph_step_host(sph_ctx *c, int64_t n, float dt, int32_t steps, const sph_stat
         SPH_CUDA_TRY(c, cudaMemcpyAsync(hs->sig[i], d.sig[i], 4 * nn, cudaMemcpyDeviceToHost, s));
     uint32_t m_host = 0;
     if (steps > 0 && (boundary_ids || boundary_count)) {
-        SPH_CUDA_TRY(c, cudaMemcpyAsync(&m_host, c->s_boundary_count, sizeof(uint32_t),
+        SPH_CUDA_TRY(c, cudaMemcpyAsync(c->h_count, c->s_boundary_count, sizeof(uint32_t),
                                         cudaMemcpyDeviceToHost, s));
         SPH_CUDA_TRY(c, cudaStreamSynchronize(s));
+        m_host = *c->h_count;
         if (boundary_ids && m_host)
             SPH_CUDA_TRY(c, cudaMemcpyAsync(boundary_ids, c->s_boundary_ids, sizeof(uint32_t) * m_host,
                                             cudaMemcpyDeviceToHost, s));
@@ -464,6 +478,21 @@ int sph_step_host(sph_ctx *c, int64_t n, float dt, int32_t steps, const sph_stat
                                         cudaMemcpyDeviceToHost, s));
     SPH_CUDA_TRY(c, cudaStreamSynchronize(s));
     return SPH_OK;
+}
+
+int sph_step_host(sph_ctx *c, int64_t n, float dt, int32_t steps, const sph_state *hs,
+                  uint32_t *boundary_ids, uint32_t *boundary_count, unsigned long long *pair_count)
+{
+    if (!n_ok(c, n) || !state_ok(hs) || steps < 0) return SPH_EINVAL;
+    const int rc = step_host_impl(c, n, dt, steps, hs, boundary_ids, boundary_count, pair_count);
+    if (rc != SPH_OK) {
+        // a failure after the copies were enqueued: do not return while either stream may still
+        // read or write the caller's host buffers, and leave no pending wait for a later sph_step
+        c->wait_before_reorder = nullptr;
+        if (c->host_streams_ready) cudaStreamSynchronize(c->copy_stream);
+        cudaStreamSynchronize(c->stream);
+    }
+    return rc;
 }
 
 int sph_enable_timing(sph_ctx *c, int32_t on)

@@ -72,6 +72,7 @@ struct sph_ctx {
     cudaStream_t copy_stream;
     cudaEvent_t ev_posm, ev_rest;
     bool host_streams_ready;
+    uint32_t *h_count;           // pinned host word: landing place of the boundary count (sph_step_host)
     cudaEvent_t wait_before_reorder;
 
     // ---- scratch (device) ----
@@ -127,7 +128,9 @@ __device__ __forceinline__ uint32_t bucket_coord(float x, float o, float inv, in
     // fp32 sequence pinned by reading S2: sub, mul (no contraction possible), then floor and clamp.
     // floor + clamp + conversion are exact operations, so they are done as ONE conversion
     // (round towards minus infinity, saturating; NaN -> 0) and two integer clamps: the same integer
-    // as clamp(floorf(u), 0, n - 1) of the oracle for every input, in 5 instead of 9 instructions.
+    // as the oracle's clamp(floorf(u), 0, n - 1) for every finite input as long as n - 1 is exact in
+    // fp32 (sph_create refuses dims above 2^24); 5 instead of 9 instructions.  A NaN position is
+    // outside the contract (sph.h: "unspecified hash").
     const float t = __fsub_rn(x, o);
     const float u = __fmul_rn(t, inv);
     const int i = __float2int_rd(u);

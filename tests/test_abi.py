@@ -74,3 +74,15 @@ def test_product_never_imports_the_oracle():
                 code = line.split("#")[0]
                 assert not re.search(r"^\s*(import|from)\s+paper_2310_03596_b200", code), (f, line)
                 assert not re.search(r'#include\s+"(sph\.h|.*csrc)', line), (f, line)
+
+
+def test_create_refuses_dims_whose_coordinates_are_not_exact_in_fp32(lib):
+    """dims[a] > 2^24: clamp(floorf(u), 0, n - 1) is no longer the same in fp32 and in integers
+    (the argument checks come before any CUDA call, so this runs without a GPU)."""
+    from paper_2310_03596_b200 import sph
+    p = sph._Params()
+    p.h, p.K, p.G, p.n_owners = 1.0, 1.0, 0.5, 1
+    p.dims[0], p.dims[1], p.dims[2] = (1 << 24) + 1, 1, 1
+    h = C.c_void_p()
+    lib.sph_create.restype = C.c_int
+    assert lib.sph_create(C.byref(h), C.byref(p), C.c_int64(4), None) == sph.SPH_EINVAL

@@ -183,18 +183,19 @@ def test_config2_full_size(sph, oracle):
 @pytest.mark.skipif(os.environ.get("SPH_SKIP_64M") == "1", reason="SPH_SKIP_64M=1")
 def test_config4_full_size(sph, oracle):
     """configs[4], 64 M particles (the maximum size; 22-bit keys, 7 813 onesweep tiles): all 20
-    steps with a full re-hash, re-sort, comm hash and compaction each; integers and floats compared
-    on the first, the middle and the last step (reading S20 for configs[3], [4])."""
-    _fullsize_case(sph, oracle, 4, int_steps=(1, 10, 20), float_steps=(1, 10, 20),
+    steps with a full re-hash, re-sort, comm hash and compaction each; every integer product
+    compared on EVERY step, the floats on the first, the middle and the last step (reading S20 for
+    configs[3], [4])."""
+    _fullsize_case(sph, oracle, 4, int_steps=range(1, 21), float_steps=(1, 10, 20),
                    expect_boundary=(0.999, 1.0))
 
 
 @pytest.mark.skipif(os.environ.get("SPH_SKIP_22M") == "1", reason="SPH_SKIP_22M=1")
 def test_config3_full_size(sph, oracle):
     """configs[3], the irregular geometry as stated (22.0 M particles: plate + 8 cylinders, long
-    runs of empty buckets, 16 owners by recursive coordinate bisection): all 10 steps, compared on
-    steps 1, 5, 10."""
-    _fullsize_case(sph, oracle, 3, int_steps=(1, 5, 10), float_steps=(1, 5, 10),
+    runs of empty buckets, 16 owners by recursive coordinate bisection): all 10 steps, integers
+    compared on every step, floats on steps 1, 5, 10."""
+    _fullsize_case(sph, oracle, 3, int_steps=range(1, 11), float_steps=(1, 5, 10),
                    expect_boundary=(0.05, 0.35))
 
 

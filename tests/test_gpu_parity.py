@@ -245,6 +245,9 @@ def test_error_codes(sph):
         sph.Context([0, 0, 0], [4, 4, 4], 1.3, n_owners=33, max_n=10)
     with pytest.raises(sph.SphError):
         sph.Context([0, 0, 0], [2048, 2048, 2048], 1.3, max_n=10)
+    with pytest.raises(sph.SphError):
+        sph.Context([0, 0, 0], [(1 << 24) + 1, 1, 1], 1.3, max_n=10)   # coordinate not exact in fp32
+    sph.Context([0, 0, 0], [1 << 24, 1, 1], 1.3, max_n=10).close()
     ctx = sph.Context([0, 0, 0], [4, 4, 4], 1.3, max_n=8)
     with pytest.raises(sph.SphError):
         ctx.sph_hash(torch.zeros((9, 4), device="cuda"))       # n > max_n
@@ -556,6 +559,25 @@ def test_varh_scaled_config_many_tiles_and_split_passes(sph, oracle):
     assert res[1][1] + res[2][1] == res[0][1]
     for name in ("drho", "acc", "dsig"):
         assert np.abs(res[1][0][name] + res[2][0][name] - res[0][0][name]).max() <= parity.RATE_TOL * scale[name]
+    # both passes from ONE search with per-particle lengths (sph_interact_ef, sorted_h != NULL),
+    # tiled and direct kernel: each rate set against orc_interact_varh(which = 1 / 2), counts exact
+    # against the split calls above
+    for flags in (0, 1):
+        c2 = ctx if flags == 0 else sph.Context.for_workload(w, flags=1)
+        e, f, pcs = c2.sph_interact_ef(sst, sh, cs, ce, sorted_h=sh_h)
+        torch.cuda.synchronize()
+        pcs = pcs.cpu().numpy()
+        assert int(pcs[0]) == res[1][1] and int(pcs[1]) == res[2][1], (flags, pcs, res[1][1], res[2][1])
+        for which, got_t in ((1, e), (2, f)):
+            ref = oracle.interact_varh(sp, sv, ss, hp[p], parity.u32(sh), w.dims, parity.u32(cs), parity.u32(ce),
+                                       w.h, w.K, w.G, owner=so, which=which)
+            got = {"drho": got_t[0].cpu().numpy(), "acc": got_t[1].cpu().numpy()[:, :3],
+                   "dsig": got_t[2].cpu().numpy().T}
+            for name in ("drho", "acc", "dsig"):
+                err = np.abs(got[name] - getattr(ref, name)).max() / scale[name]
+                assert err <= parity.RATE_TOL, ("ef", flags, which, name, err)
+        if c2 is not ctx:
+            c2.close()
     ctx.close()
 
 
