@@ -39,6 +39,8 @@ def _load():
     lib.orc_boundary.restype = i64
     lib.orc_pack_boundary.argtypes = [i64, i64, vp, vp, C.c_int32] + [vp] * 9
     lib.orc_pack_boundary.restype = None
+    lib.orc_pack_destinations.argtypes = [i64, vp, vp, vp, vp, vp, vp, C.c_int32, vp, vp, i64]
+    lib.orc_pack_destinations.restype = i64
     lib.orc_balance.argtypes = [i64, vp, vp, C.c_int32, C.c_int32, vp]
     lib.orc_balance.restype = i64
     lib.orc_balance_types.argtypes = [i64, vp, vp, vp, C.c_int32, C.c_int32, C.c_int32, f64, vp]
@@ -188,6 +190,29 @@ def pack_boundary(boundary_ids, owner, n_owners: int, posm, velr, sig) -> Packed
     _load().orc_pack_boundary(n, m, _p(boundary_ids), _p(owner), int(n_owners), _p(posm), _p(velr),
                               _p(sig), _p(off), _p(ids), _p(pp), _p(pv), _p(ps), _p(po))
     return PackedBoundary(off, ids, pp, pv, ps, po)
+
+
+def pack_destinations(sorted_hash, sorted_owner, perm, dims, cell_start, cell_end, n_owners: int):
+    """Per-destination send lists (sph_oracle.c O5c, reading D1): returns
+    (dest_offsets [n_owners + 1] u32, dest_ids [total] u32); list g = dest_ids[offsets[g]:offsets[g + 1]]
+    = ids, in (hash, id) order, of the particles not owned by g that have a particle of g in their
+    27-bucket stencil.  All inputs in sorted order."""
+    sorted_hash = _c(sorted_hash, np.uint32)
+    sorted_owner = _c(sorted_owner, np.int32)
+    perm = _c(perm, np.uint32)
+    dims = _c(dims, np.int32)
+    cell_start = _c(cell_start, np.uint32)
+    cell_end = _c(cell_end, np.uint32)
+    n = sorted_hash.shape[0]
+    off = np.zeros(n_owners + 1, np.uint32)
+    lib = _load()
+    total = lib.orc_pack_destinations(n, _p(sorted_hash), _p(sorted_owner), _p(perm), _p(dims), _p(cell_start),
+                                      _p(cell_end), int(n_owners), _p(off), None, 0)
+    ids = np.empty(max(total, 1), np.uint32)
+    t2 = lib.orc_pack_destinations(n, _p(sorted_hash), _p(sorted_owner), _p(perm), _p(dims), _p(cell_start),
+                                   _p(cell_end), int(n_owners), _p(off), _p(ids), total)
+    assert t2 == total
+    return off, ids[:total]
 
 
 @dataclass

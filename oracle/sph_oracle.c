@@ -205,6 +205,52 @@ void orc_pack_boundary(int64_t n, int64_t m, const uint32_t *boundary_ids, const
 }
 
 /* ------------------------------------------------------------------------------------------
+ * O5c  Per-DESTINATION send lists (second half; PAPER.md:23 step d "Each
+ * GPU broadcasts its MGPU boundary particle data to the other GPUs").  The paper sends every
+ * boundary particle to every other GPU; GPU g only ever uses a foreign particle that lies in the
+ * own or a surrounding bucket of one of ITS particles (PAPER.md:25 step f searches the same 27
+ * buckets).  Reading D1: particle k is on the list of destination g iff its owner
+ * is not g and a particle owned by g lies in the 27-bucket stencil of k's bucket (bucket-level
+ * test as for the communication hash, readings S9 / S10).  Each list holds particle ids in the
+ * (hash, id) order of the sorted array; lists are stored back to back by ascending g,
+ * dest_offsets[g] = entries of the lists before g, dest_offsets[n_owners] = total.
+ * Plain per-destination, per-particle definition; all arrays in sorted order (index k).
+ * dest_ids may be NULL (count only); entries beyond `cap` are counted but not stored.
+ * Returns the total number of entries.
+ * ---------------------------------------------------------------------------------------- */
+int64_t orc_pack_destinations(int64_t n, const uint32_t *sorted_hash, const int32_t *sorted_owner,
+                              const uint32_t *perm, const int32_t *dims, const uint32_t *cell_start,
+                              const uint32_t *cell_end, int32_t n_owners, uint32_t *dest_offsets,
+                              uint32_t *dest_ids, int64_t cap)
+{
+    const int64_t nx = dims[0], ny = dims[1], nz = dims[2];
+    int64_t total = 0;
+    for (int32_t g = 0; g < n_owners; ++g) {
+        dest_offsets[g] = (uint32_t)total;
+        for (int64_t k = 0; k < n; ++k) {
+            if (sorted_owner[k] == g) continue; /* a GPU does not send to itself */
+            const int64_t hsh = sorted_hash[k];
+            const int64_t cx = hsh % nx, cy = (hsh / nx) % ny, cz = hsh / (nx * ny);
+            int found = 0;
+            for (int64_t dz = -1; dz <= 1 && !found; ++dz)
+                for (int64_t dy = -1; dy <= 1 && !found; ++dy)
+                    for (int64_t dx = -1; dx <= 1 && !found; ++dx) {
+                        const int64_t x = cx + dx, y = cy + dy, z = cz + dz;
+                        if (x < 0 || x >= nx || y < 0 || y >= ny || z < 0 || z >= nz) continue;
+                        const int64_t c = x + nx * (y + ny * z);
+                        for (uint32_t j = cell_start[c]; j < cell_end[c]; ++j)
+                            if (sorted_owner[j] == g) { found = 1; break; }
+                    }
+            if (!found) continue;
+            if (dest_ids && total < cap) dest_ids[total] = perm[k];
+            ++total;
+        }
+    }
+    dest_offsets[n_owners] = (uint32_t)total;
+    return total;
+}
+
+/* ------------------------------------------------------------------------------------------
  * O6  Kernel (BASELINE.json configs[0]: "Wendland C2 kernel with support 2h"; reading S14).
  * q = r/h;  W = alpha (1 - q/2)^4 (1 + 2q),  alpha = 21 / (16 pi h^3)   for q < 2, else 0.
  * grad_i W_ij = F(r) x_ij with F(r) = (dW/dr)/r = -(5 alpha / h^2) (1 - q/2)^3.

@@ -520,6 +520,71 @@ def test_pack_boundary_vs_stable_argsort_and_invariants(make):
     np.testing.assert_array_equal(pb.owner, w.owner[pb.ids])
 
 
+@pytest.mark.parametrize("owners", [("plane_x", 5.0), ("slabs", 3), ("slabs_mixed", 4, 0.02), ("rcb", 3),
+                                    ("random", 5), ("single",)])
+def test_pack_destinations_dense_checker_and_invariants(owners):
+    """O5c (PAPER.md:23 step d, reading D1): the list of destination g against a dense
+    bucket-coordinate checker written in numpy, plus what must hold whatever the layout: every list
+    in (hash, id) order, no particle sent to its own owner, union of the lists = the MGPU boundary
+    set (a particle is a boundary particle iff SOME other owner is in its stencil), never more
+    entries than the paper's broadcast-to-all (M (G - 1)), exactly that many under full mixing."""
+    w = W.lattice_block(11, 9, 10, 0.1, 79, owners=owners)
+    g_n = w.n_owners
+    r, sp, sv, ss, so = sorted_view(w)
+    off, ids = orc.pack_destinations(r.sorted_hash, so, r.perm, w.dims, r.cell_start, r.cell_end, g_n)
+    assert off[0] == 0 and off[-1] == ids.size and (np.diff(off.astype(np.int64)) >= 0).all()
+    c = bucket_coords_f32(w.posm, w.origin, w.dims, w.h)                     # id order
+    near = (np.abs(c[:, None, :] - c[None, :, :]) <= 1).all(-1)
+    rank = np.empty(w.n, np.int64); rank[r.perm] = np.arange(w.n)            # position in (hash, id) order
+    for g in range(g_n):
+        lst = ids[off[g]:off[g + 1]]
+        want = (w.owner != g) & (near & (w.owner[None, :] == g)).any(1)
+        np.testing.assert_array_equal(lst, r.perm[want[r.perm]], err_msg=f"destination {g}")
+        assert (w.owner[lst] != g).all()
+        assert (np.diff(rank[lst]) > 0).all()
+    np.testing.assert_array_equal(np.unique(ids), np.sort(r.boundary_ids))
+    m = r.boundary_ids.size
+    assert ids.size <= m * (g_n - 1)
+    if owners[0] == "random":
+        assert ids.size == w.n * (g_n - 1)          # PAPER.md:30 full mixing: nothing is saved
+    if owners[0] == "single":
+        assert ids.size == 0
+    if g_n == 2:
+        # two owners: what goes to g is exactly the other owner's send segment of O5b
+        pk = orc.pack_boundary(r.boundary_ids, w.owner, 2, w.posm, w.velr, w.sig)
+        np.testing.assert_array_equal(ids[off[1]:off[2]], pk.ids[pk.offsets[0]:pk.offsets[1]])
+        np.testing.assert_array_equal(ids[off[0]:off[1]], pk.ids[pk.offsets[1]:pk.offsets[2]])
+
+
+def test_pack_destinations_wide_slabs_halve_the_broadcast():
+    """Three slabs, each wider than a stencil (PAPER.md:30 'two surfaces'): every boundary particle
+    has exactly ONE foreign neighbour owner, so the per-destination lists hold M entries where the
+    paper's broadcast to all other GPUs ships 2 M; the outer slabs exchange nothing."""
+    w = W.lattice_block(40, 6, 6, 0.1, 80, owners=("slabs", 3))
+    r, sp, sv, ss, so = sorted_view(w)
+    off, ids = orc.pack_destinations(r.sorted_hash, so, r.perm, w.dims, r.cell_start, r.cell_end, 3)
+    m = r.boundary_ids.size
+    assert 0 < m < w.n and ids.size == m and np.unique(ids).size == m
+    assert (w.owner[ids[off[0]:off[1]]] == 1).all() and (w.owner[ids[off[2]:off[3]]] == 1).all()
+    assert set(w.owner[ids[off[1]:off[2]]]) == {0, 2}
+
+
+def test_pack_destinations_one_foreign_particle():
+    """One particle of owner 1 in an interior bucket: destination 1 receives exactly the owner-0
+    particles of the 27 buckets around it, destination 0 receives that one particle."""
+    w = W.lattice_block(14, 13, 12, 0.1, 78)
+    c = bucket_coords_f32(w.posm, w.origin, w.dims, w.h)
+    f = np.nonzero((c == np.array([2, 2, 2])).all(1))[0][0]
+    w.owner = np.zeros(w.n, np.int32); w.owner[f] = 1; w.n_owners = 2
+    r, sp, sv, ss, so = sorted_view(w)
+    off, ids = orc.pack_destinations(r.sorted_hash, so, r.perm, w.dims, r.cell_start, r.cell_end, 2)
+    np.testing.assert_array_equal(ids[off[0]:off[1]], [f])
+    near = (np.abs(c - c[f]) <= 1).all(1)
+    near[f] = False
+    np.testing.assert_array_equal(np.sort(ids[off[1]:off[2]]), np.nonzero(near)[0])
+    assert len(np.unique(c[ids[off[1]:off[2]]], axis=0)) == 27
+
+
 def test_pack_boundary_single_owner_is_empty():
     w = W.lattice_block(8, 8, 8, 0.1, 3, owners=("single",))
     r = orc.step(w.posm, w.velr, w.sig, w.owner, w.origin, w.dims, w.h, w.K, w.G, w.n_owners, w.dt,
