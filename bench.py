@@ -283,6 +283,35 @@ def run_ours(args, rank, world, local_rank):
                 "note": "outputs pre-allocated (no allocation inside the timed interval)"}
         del o2, bids_dev, bcnt, pk_out
 
+    # ---- NEXT-1, second half (not part of the step metric): per-destination send lists ----
+    dests = None
+    if w.n_owners > 1 and n * (w.n_owners - 1) < (1 << 30):
+        hh = ctx.sph_hash(state.posm)
+        sh_, pm_ = ctx.sph_sort(hh)
+        so_ = state.owner[pm_.long()].contiguous()
+        cs_, ce_ = ctx.sph_cell_ranges(sh_)
+        _ch, _bi, cnt_, _oc = ctx.sph_comm_hash(sh_, so_, pm_, cs_, ce_)
+        offs_, ids_ = ctx.sph_pack_destinations(sh_, so_, pm_)          # sizes the buffer (one host sync)
+        torch.cuda.synchronize(dev)
+        m_b2 = int(sph.as_u32(cnt_)[0])
+        total_d = int(sph.as_u32(offs_)[-1])
+        ts = []
+        for _ in range(5):
+            flush.zero_()
+            a_, b_ = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            a_.record()
+            ctx.sph_pack_destinations(sh_, so_, pm_, dest_ids=ids_, dest_offsets=offs_)
+            b_.record()
+            torch.cuda.synchronize(dev)
+            ts.append(a_.elapsed_time(b_))
+        bcast = m_b2 * (w.n_owners - 1)
+        dests = {"ms": round(float(np.median(ts[1:])), 4), "entries": total_d, "broadcast_entries": bcast,
+                 "entries_over_broadcast": round(total_d / bcast, 4) if bcast else None,
+                 "record_bytes_saved": 156 * (bcast - total_d),
+                 "note": "entries = sum over destinations g of the boundary particles g really needs (reading D1); "
+                         "broadcast = every boundary particle to every other owner (PAPER.md:23)"}
+        del hh, sh_, pm_, so_, cs_, ce_, _ch, _bi, cnt_, _oc, offs_, ids_
+
     # ---- NEXT-3 (not part of the step metric): steps e / f as separate interaction passes ----
     split = None
     if w.n_owners > 1:
@@ -435,6 +464,8 @@ def run_ours(args, rank, world, local_rank):
         pack["gbs"] = round(pack["bytes_per_boundary_particle"] * pack["boundary_particles"] / (pack["ms"] * 1e-3) / 1e9, 1)
         pack["hbm_frac"] = round(pack["gbs"] / peaks["hbm_gbs"], 3)
         line["next1_pack_boundary"] = pack
+    if dests:
+        line["next1_pack_destinations"] = dests
     if split:
         line["next3_split_passes"] = split
     if bal:

@@ -43,7 +43,7 @@ extern "C" {
 #define SPH_EINVAL   -1   /* null pointer, n < 0, n > max_n, bad params                         */
 #define SPH_ECUDA    -2   /* a CUDA runtime call or launch failed (see sph_last_cuda_error)     */
 #define SPH_ENOMEM   -3   /* scratch allocation failed                                           */
-#define SPH_ELIMIT   -4   /* size beyond the fixed capacity of sph_comm_hash_noalloc             */
+#define SPH_ELIMIT   -4   /* size beyond a fixed capacity stated at the entry point's declaration */
 
 #define SPH_GARBAGE_HASH 0xFFFFFFFFu  /* PAPER.md:17 "some garbage collector hash" (reading S8) */
 #define SPH_MAX_OWNERS   32           /* paper's envelope is <= 16 GPUs           */
@@ -184,6 +184,25 @@ int sph_step(sph_ctx *ctx, int64_t n, float dt, const sph_state *state,
 int sph_pack_boundary(sph_ctx *ctx, int64_t n, int64_t m, const sph_state *state,
                       const uint32_t *boundary_ids, uint32_t *owner_offsets, uint32_t *packed_ids,
                       const sph_state *packed);
+
+/* NEXT-1, second half -- per-DESTINATION send lists.  Step d of the paper ships every
+ * MGPU boundary particle to every other GPU ("Each GPU broadcasts its MGPU boundary
+ * particle data to the other GPUs"); GPU g, however, only uses a foreign particle that lies in the
+ * own or a surrounding bucket of one of its particles (step f searches those 27 buckets,
+ * PAPER.md:25).  Reading D1: particle k is on the list of destination g iff
+ * owner_k != g and a particle owned by g lies in the 27-bucket stencil of k's bucket (bucket-level
+ * test, out-of-grid buckets skipped, as for the communication hash).  The union of the lists is the
+ * boundary set; their total length is at most M (n_owners - 1), the size of the broadcast, and far
+ * less for compact decompositions (three wide slabs: half).
+ * In: sorted_hash, sorted_owner, perm dev [n] (sorted order, as for sph_comm_hash; no cell tables).
+ * Out: dest_offsets dev [n_owners + 1]: list g = dest_ids[dest_offsets[g] .. dest_offsets[g + 1]),
+ * dest_offsets[n_owners] = total number of entries; dest_ids dev, capacity `cap` entries, or NULL to
+ * get the offsets only (size the buffer, then call again): particle ids (perm values), each list
+ * in (hash, id) order.  Entries beyond cap are not written (compare the total with cap after
+ * synchronising).  Limit: n (n_owners - 1) must be below 2^30 (SPH_ELIMIT otherwise: the scan
+ * carries 30-bit prefixes).  Enqueues only; not part of sph_step. */
+int sph_pack_destinations(sph_ctx *ctx, int64_t n, const uint32_t *sorted_hash, const int32_t *sorted_owner,
+                          const uint32_t *perm, uint32_t *dest_offsets, uint32_t *dest_ids, int64_t cap);
 
 /* NEXT-2 -- one sweep of the communication-load balancing heuristic on the owner
  * labels, single particle type (section III.A; the paper runs it every 20 integration

@@ -209,7 +209,7 @@ void orc_pack_boundary(int64_t n, int64_t m, const uint32_t *boundary_ids, const
  * GPU broadcasts its MGPU boundary particle data to the other GPUs").  The paper sends every
  * boundary particle to every other GPU; GPU g only ever uses a foreign particle that lies in the
  * own or a surrounding bucket of one of ITS particles (PAPER.md:25 step f searches the same 27
- * buckets).  Reading D1 (DESIGN.md 6.4): particle k is on the list of destination g iff its owner
+ * buckets).  Reading D1 (DESIGN.md 6.3.1): particle k is on the list of destination g iff its owner
  * is not g and a particle owned by g lies in the 27-bucket stencil of k's bucket (bucket-level
  * test as for the communication hash, readings S9 / S10).  Each list holds particle ids in the
  * (hash, id) order of the sorted array; lists are stored back to back by ascending g,

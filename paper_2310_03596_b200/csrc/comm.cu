@@ -60,6 +60,9 @@ owner_mask_kernel(int64_t n, const uint32_t *__restrict__ sorted_hash,
 // each (54 loads for 4 buckets instead of 108) and OR-ed with a sliding window.
 constexpr int kFlagCells = 4;
 
+// kMaskOut = false: flag_count[c] = flagged particle count of bucket c (stage 3);
+// kMaskOut = true:  flag_count[c] = the stencil's owner mask itself (per-destination lists, NEXT-1).
+template <bool kMaskOut>
 __global__ void __launch_bounds__(256)
 stencil_flag_kernel(Grid g, const uint32_t *__restrict__ cell_mask, const uint32_t *__restrict__ cs,
                     const uint32_t *__restrict__ ce, uint32_t *__restrict__ flag_count)
@@ -95,8 +98,12 @@ stencil_flag_kernel(Grid g, const uint32_t *__restrict__ cell_mask, const uint32
         if (x >= g.nx) break;
         const uint32_t m = col[i] | col[i + 1] | col[i + 2];
         const uint32_t c = row0 + (uint32_t)x;
-        // an empty bucket contributes no particles whatever its stencil holds
-        flag_count[c] = (__popc(m) >= 2) ? (ce[c] - cs[c]) : 0u;
+        if (kMaskOut) {
+            flag_count[c] = m;
+        } else {
+            // an empty bucket contributes no particles whatever its stencil holds
+            flag_count[c] = (__popc(m) >= 2) ? (ce[c] - cs[c]) : 0u;
+        }
     }
 }
 
@@ -225,8 +232,8 @@ int launch_comm_hash(sph_ctx *c, int64_t n, const uint32_t *sorted_hash, const i
     SPH_CHECK_LAUNCH(c);
     {
         const int64_t groups = (int64_t)((c->grid.nx + kFlagCells - 1) / kFlagCells) * c->grid.ny * c->grid.nz;
-        stencil_flag_kernel<<<div_up(groups, 256), 256, 0, c->stream>>>(c->grid, c->cell_mask, cs, ce,
-                                                                        c->cell_flag_count);
+        stencil_flag_kernel<false><<<div_up(groups, 256), 256, 0, c->stream>>>(c->grid, c->cell_mask, cs, ce,
+                                                                               c->cell_flag_count);
     }
     SPH_CHECK_LAUNCH(c);
     int rc = launch_scan_exclusive(c, cells, c->cell_flag_count, c->cell_offset, boundary_count);
@@ -234,6 +241,129 @@ int launch_comm_hash(sph_ctx *c, int64_t n, const uint32_t *sorted_hash, const i
     comm_hash_compact_kernel<<<div_up(div_up(n, kCompItems), 256), 256, 0, c->stream>>>(
         n, sorted_hash, sorted_owner, perm, cs, c->cell_flag_count, c->cell_offset, comm_hash,
         boundary_ids, owner_counts, c->params.n_owners);
+    SPH_CHECK_LAUNCH(c);
+    return SPH_OK;
+}
+
+// ---- NEXT-1, second half: per-DESTINATION send lists (PAPER.md:23 step d; reading D1) --------
+// Particle k goes to destination g iff g != owner_k and bit g is set in the owner mask of the
+// 27-bucket stencil of k's bucket -- the mask stencil_flag_kernel ORs together anyway.  List g
+// holds the ids of its particles in sorted order, so the whole product is a stable multi-way
+// split in which one particle may enter several lists:
+//   pass 1  per tile of 256 sorted particles, the number of entries for each destination
+//           (warp ballots), stored destination-major: counts[g * tiles + tile];
+//   scan    one exclusive scan over that array gives every (destination, tile) its first slot,
+//           the lists back to back by ascending g;
+//   pass 2  the same ballots again give each entry its rank inside the tile.
+constexpr int kDestThreads = 256;
+
+__device__ __forceinline__ uint32_t dest_bits(int64_t k, int64_t n, const uint32_t *__restrict__ sorted_hash,
+                                              const int32_t *__restrict__ sorted_owner,
+                                              const uint32_t *__restrict__ stencil_mask)
+{
+    if (k >= n) return 0u;
+    return __ldg(stencil_mask + sorted_hash[k]) & ~(1u << (sorted_owner[k] & 31));
+}
+
+__global__ void __launch_bounds__(kDestThreads)
+dest_count_kernel(int64_t n, const uint32_t *__restrict__ sorted_hash, const int32_t *__restrict__ sorted_owner,
+                  const uint32_t *__restrict__ stencil_mask, uint32_t *__restrict__ counts, uint32_t tiles,
+                  int n_owners)
+{
+    __shared__ uint32_t s_cnt[kDestThreads / 32][SPH_MAX_OWNERS];
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    const int64_t k = (int64_t)blockIdx.x * kDestThreads + threadIdx.x;
+    const uint32_t bits = dest_bits(k, n, sorted_hash, sorted_owner, stencil_mask);
+    uint32_t mine = 0u;   // lane g keeps the warp's count for destination g
+    uint32_t any = __reduce_or_sync(0xffffffffu, bits);
+    while (any) {
+        const int g = __ffs(any) - 1;
+        any &= any - 1;
+        const uint32_t votes = __ballot_sync(0xffffffffu, (bits >> g) & 1u);
+        if (lane == g) mine = __popc(votes);
+    }
+    s_cnt[warp][lane] = mine;
+    __syncthreads();
+    if (threadIdx.x < n_owners) {
+        uint32_t tot = 0;
+#pragma unroll
+        for (int w = 0; w < kDestThreads / 32; ++w) tot += s_cnt[w][threadIdx.x];
+        counts[(size_t)threadIdx.x * tiles + blockIdx.x] = tot;
+    }
+}
+
+__global__ void __launch_bounds__(kDestThreads)
+dest_scatter_kernel(int64_t n, const uint32_t *__restrict__ sorted_hash, const int32_t *__restrict__ sorted_owner,
+                    const uint32_t *__restrict__ perm, const uint32_t *__restrict__ stencil_mask,
+                    const uint32_t *__restrict__ offsets, uint32_t tiles, int n_owners,
+                    uint32_t *__restrict__ dest_offsets, uint32_t *__restrict__ dest_ids, uint32_t cap)
+{
+    __shared__ uint32_t s_cnt[kDestThreads / 32][SPH_MAX_OWNERS];
+    __shared__ uint32_t s_base[kDestThreads / 32][SPH_MAX_OWNERS];
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    const int64_t k = (int64_t)blockIdx.x * kDestThreads + threadIdx.x;
+    const uint32_t bits = dest_bits(k, n, sorted_hash, sorted_owner, stencil_mask);
+    const uint32_t id = k < n ? perm[k] : 0u;
+    const uint32_t warp_any = __reduce_or_sync(0xffffffffu, bits);
+    uint32_t mine = 0u;
+    for (uint32_t any = warp_any; any;) {
+        const int g = __ffs(any) - 1;
+        any &= any - 1;
+        const uint32_t votes = __ballot_sync(0xffffffffu, (bits >> g) & 1u);
+        if (lane == g) mine = __popc(votes);
+    }
+    s_cnt[warp][lane] = mine;
+    __syncthreads();
+    if (threadIdx.x < n_owners) {   // first slot of every warp of this tile in list g
+        uint32_t run = offsets[(size_t)threadIdx.x * tiles + blockIdx.x];
+        if (blockIdx.x == 0) dest_offsets[threadIdx.x] = run;   // list g starts where its tile 0 does
+#pragma unroll
+        for (int w = 0; w < kDestThreads / 32; ++w) {
+            s_base[w][threadIdx.x] = run;
+            run += s_cnt[w][threadIdx.x];
+        }
+    }
+    __syncthreads();
+    if (!dest_ids) return;
+    for (uint32_t any = warp_any; any;) {
+        const int g = __ffs(any) - 1;
+        any &= any - 1;
+        const uint32_t votes = __ballot_sync(0xffffffffu, (bits >> g) & 1u);
+        if ((bits >> g) & 1u) {
+            const uint32_t slot = s_base[warp][g] + __popc(votes & lanemask_lt());
+            if (slot < cap) dest_ids[slot] = id;
+        }
+    }
+}
+
+int launch_pack_destinations(sph_ctx *c, int64_t n, const uint32_t *sorted_hash, const int32_t *sorted_owner,
+                             const uint32_t *perm, uint32_t *dest_offsets, uint32_t *dest_ids, int64_t cap)
+{
+    const int G = c->params.n_owners;
+    if (n == 0) {
+        SPH_CUDA_TRY(c, cudaMemsetAsync(dest_offsets, 0, sizeof(uint32_t) * (G + 1), c->stream));
+        return SPH_OK;
+    }
+    const uint32_t cells = c->grid.n_cells;
+    const uint32_t tiles = (uint32_t)div_up(n, kDestThreads);
+    uint32_t *counts = c->dest_counts, *offsets = c->dest_counts + (size_t)G * tiles;
+    uint32_t *stencil_mask = c->cell_flag_count;   // stage 3's per-bucket scratch, free outside sph_comm_hash
+    SPH_CUDA_TRY(c, cudaMemsetAsync(c->cell_mask, 0, sizeof(uint32_t) * cells, c->stream));
+    owner_mask_kernel<<<div_up(div_up(n, kMaskItems), 256), 256, 0, c->stream>>>(n, sorted_hash, sorted_owner, c->cell_mask);
+    SPH_CHECK_LAUNCH(c);
+    {
+        const int64_t groups = (int64_t)((c->grid.nx + kFlagCells - 1) / kFlagCells) * c->grid.ny * c->grid.nz;
+        stencil_flag_kernel<true><<<div_up(groups, 256), 256, 0, c->stream>>>(c->grid, c->cell_mask, nullptr, nullptr,
+                                                                              stencil_mask);
+    }
+    SPH_CHECK_LAUNCH(c);
+    dest_count_kernel<<<tiles, kDestThreads, 0, c->stream>>>(n, sorted_hash, sorted_owner, stencil_mask, counts, tiles, G);
+    SPH_CHECK_LAUNCH(c);
+    int rc = launch_scan_exclusive(c, (int64_t)G * tiles, counts, offsets, dest_offsets + G);
+    if (rc != SPH_OK) return rc;
+    const uint32_t cap32 = (uint32_t)(cap > 0xffffffffll ? 0xffffffffll : cap);
+    dest_scatter_kernel<<<tiles, kDestThreads, 0, c->stream>>>(n, sorted_hash, sorted_owner, perm, stencil_mask, offsets,
+                                                               tiles, G, dest_offsets, dest_ids, cap32);
     SPH_CHECK_LAUNCH(c);
     return SPH_OK;
 }

@@ -48,6 +48,7 @@ void carve(sph_ctx *c, char *base, size_t *total)
     c->cell_flag_count = k.take<uint32_t>(cells);
     c->cell_offset = k.take<uint32_t>(cells);
     c->scan_status = k.take<uint32_t>(scan_tiles);
+    c->dest_counts = k.take<uint32_t>(2 * (size_t)c->params.n_owners * ((n + 255) / 256));
     c->s_hash = k.take<uint32_t>(n);
     c->s_sorted_hash = k.take<uint32_t>(n);
     c->s_perm = k.take<uint32_t>(n);
@@ -304,6 +305,15 @@ int sph_interact_ef(sph_ctx *c, int64_t n, const sph_state *sorted, const float 
                            0.f, 3, sorted_h, drho_f, acc_f, dsig_f);
 }
 
+int sph_pack_destinations(sph_ctx *c, int64_t n, const uint32_t *sorted_hash, const int32_t *sorted_owner,
+                          const uint32_t *perm, uint32_t *dest_offsets, uint32_t *dest_ids, int64_t cap)
+{
+    if (!n_ok(c, n) || !dest_offsets || cap < 0) return SPH_EINVAL;
+    if (n > 0 && (!sorted_hash || !sorted_owner || !perm)) return SPH_EINVAL;
+    if (n * (int64_t)(c->params.n_owners - 1) >= (1ll << 30)) return SPH_ELIMIT;   // 30-bit scan prefixes
+    return launch_pack_destinations(c, n, sorted_hash, sorted_owner, perm, dest_offsets, dest_ids, cap);
+}
+
 int sph_integrate(sph_ctx *c, int64_t n, float dt, const sph_state *in, const float *drho,
                   const float *acc, const float *const dsig[6], const sph_state *out)
 {
@@ -538,7 +548,7 @@ const char *sph_strerror(int code)
     case SPH_EINVAL: return "invalid argument";
     case SPH_ECUDA: return "CUDA error";
     case SPH_ENOMEM: return "out of device memory";
-    case SPH_ELIMIT: return "grid has more buckets than the built-in scratch of sph_comm_hash_noalloc holds (SPH_NOALLOC_MAX_CELLS)";
+    case SPH_ELIMIT: return "size beyond a fixed capacity of the entry point (sph_comm_hash_noalloc: more than SPH_NOALLOC_MAX_CELLS buckets; sph_pack_destinations: n (n_owners - 1) >= 2^30)";
     default: return "unknown error";
     }
 }

@@ -86,6 +86,7 @@ struct sph_ctx {
     uint32_t *cell_flag_count;                // [cells] flagged particle count per bucket
     uint32_t *cell_offset;                    // [cells] exclusive scan of the above
     uint32_t *scan_status;                    // [scan tiles]
+    uint32_t *dest_counts;                    // [2][n_owners][ceil(n / 256)] per-destination tile counts and their scan (NEXT-1)
     // step-internal products (used when the caller passes NULL)
     uint32_t *s_hash, *s_sorted_hash, *s_perm, *s_cell_start, *s_cell_end, *s_comm_hash;
     uint32_t *s_boundary_ids, *s_boundary_count, *s_owner_counts;
@@ -158,6 +159,8 @@ int launch_comm_hash(sph_ctx *c, int64_t n, const uint32_t *sorted_hash, const i
                      const uint32_t *perm, const uint32_t *cs, const uint32_t *ce,
                      uint32_t *comm_hash, uint32_t *boundary_ids, uint32_t *boundary_count,
                      uint32_t *owner_counts);
+int launch_pack_destinations(sph_ctx *c, int64_t n, const uint32_t *sorted_hash, const int32_t *sorted_owner,
+                             const uint32_t *perm, uint32_t *dest_offsets, uint32_t *dest_ids, int64_t cap);
 int launch_interact(sph_ctx *c, int64_t n, const sph_state *sorted, const uint32_t *sorted_hash,
                     const uint32_t *cs, const uint32_t *ce, float *drho, float *acc,
                     float *const dsig[6], unsigned long long *pair_count,

@@ -32,7 +32,7 @@ EXPORTS = (
     "sph_create", "sph_destroy", "sph_hash", "sph_sort", "sph_reorder", "sph_cell_ranges",
     "sph_comm_hash", "sph_interact", "sph_integrate", "sph_step", "sph_step_host", "sph_pack_boundary",
     "sph_interact_split", "sph_interact_varh", "sph_step_varh", "sph_interact_ef", "sph_balance", "sph_balance_types", "sph_enable_timing", "sph_get_timing", "sph_launch_count", "sph_strerror",
-    "sph_last_cuda_error", "sph_comm_hash_noalloc",
+    "sph_last_cuda_error", "sph_comm_hash_noalloc", "sph_pack_destinations",
 )
 
 
@@ -84,6 +84,7 @@ def load_library() -> C.CDLL:
     lib.sph_balance.argtypes = [vp, i64, vp, vp, i32, vp, vp]
     lib.sph_balance_types.argtypes = [vp, i64, vp, vp, vp, i32, C.c_double, i32, vp, vp]
     lib.sph_pack_boundary.argtypes = [vp, i64, i64, sp, vp, vp, vp, sp]
+    lib.sph_pack_destinations.argtypes = [vp, i64, vp, vp, vp, vp, vp, i64]
     lib.sph_enable_timing.argtypes = [vp, i32]
     lib.sph_get_timing.argtypes = [vp, C.POINTER(f32 * 8)]
     lib.sph_launch_count.argtypes = [vp]
@@ -444,6 +445,25 @@ class Context:
                                              offs.data_ptr(), ids.data_ptr(), C.byref(b)), "sph_pack_boundary")
         return offs, ids[:m], State(packed.posm[:m], packed.velr[:m], packed.sig[:, :m], packed.owner[:m])
 
+    def sph_pack_destinations(self, sorted_hash, sorted_owner, perm, dest_ids: torch.Tensor | None = None,
+                              dest_offsets: torch.Tensor | None = None):
+        """Per-destination send lists (NEXT-1; reading D1).  Without `dest_ids` the call
+        is made twice: once for the offsets (the total is read back, a host sync), once to fill a
+        buffer of exactly that size.  With `dest_ids` (int32, capacity entries) it only enqueues.
+        Returns (dest_offsets [n_owners + 1], dest_ids)."""
+        n = int(sorted_hash.shape[0])
+        offs = dest_offsets if dest_offsets is not None else self._i32(self.n_owners + 1)
+        args = (self.handle, n, _ptr(sorted_hash), _ptr(sorted_owner), _ptr(perm), offs.data_ptr())
+        if dest_ids is None:
+            self._chk(self.lib.sph_pack_destinations(*args, None, 0), "sph_pack_destinations")
+            total = int(as_u32(offs)[-1])
+            dest_ids = self._i32(max(total, 1))
+            self._chk(self.lib.sph_pack_destinations(*args, dest_ids.data_ptr(), total), "sph_pack_destinations")
+            return offs, dest_ids[:total]
+        self._chk(self.lib.sph_pack_destinations(*args, dest_ids.data_ptr(), int(dest_ids.numel())),
+                  "sph_pack_destinations")
+        return offs, dest_ids
+
     def sph_step_host(self, host_state: State, dt, steps=1, boundary_ids: np.ndarray | None = None):
         """End to end with HOST buffers (pinned recommended): H2D, `steps` iterations, D2H, sync.
         Returns (boundary_count, pair_count) as Python ints; host_state is updated in place."""
@@ -509,3 +529,4 @@ def sph_step_host(ctx, *a, **k): return ctx.sph_step_host(*a, **k)
 def sph_pack_boundary(ctx, *a, **k): return ctx.sph_pack_boundary(*a, **k)
 def sph_balance(ctx, *a, **k): return ctx.sph_balance(*a, **k)
 def sph_balance_types(ctx, *a, **k): return ctx.sph_balance_types(*a, **k)
+def sph_pack_destinations(ctx, *a, **k): return ctx.sph_pack_destinations(*a, **k)

@@ -298,3 +298,27 @@ def test_split_passes_config1_full_size(sph, oracle):
     for name in ("drho", "acc", "dsig"):
         assert np.abs(res[1][0][name] + res[2][0][name] - single[name]).max() <= parity.RATE_TOL * scale[name]
     ctx.close()
+
+
+def test_pack_destinations_config1_full_size(sph, oracle):
+    """sph_pack_destinations (PAPER.md:23 step d, reading D1) on configs[1] (1 M particles, 4 slabs,
+    3 907 tiles of 256) after 3 steps, bit-exact against orc_pack_destinations; with slabs wider
+    than a stencil every boundary particle has one destination: a third of the broadcast."""
+    w = wl.config(1)
+    ctx = sph.Context.for_workload(w)
+    state = sph.State.from_numpy(w.posm, w.velr, w.sig, w.owner)
+    for _ in range(3):
+        ctx.sph_step(state, w.dt)
+    sh, perm = ctx.sph_sort(ctx.sph_hash(state.posm))
+    so = state.owner[perm.long()].contiguous()
+    cs, ce = ctx.sph_cell_ranges(sh)
+    offs, ids = ctx.sph_pack_destinations(sh, so, perm)
+    _, _, cnt, _ = ctx.sph_comm_hash(sh, so, perm, cs, ce)
+    torch.cuda.synchronize()
+    ref_off, ref_ids = oracle.pack_destinations(parity.u32(sh), so.cpu().numpy(), parity.u32(perm), w.dims,
+                                                parity.u32(cs), parity.u32(ce), w.n_owners)
+    np.testing.assert_array_equal(parity.u32(offs), ref_off)
+    np.testing.assert_array_equal(parity.u32(ids), ref_ids)
+    m = int(parity.u32(cnt)[0])
+    assert ref_ids.size == m and np.unique(ref_ids).size == m       # one destination per boundary particle
+    ctx.close()

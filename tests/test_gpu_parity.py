@@ -670,3 +670,51 @@ def test_balance_three_owner_golden_example_on_the_gpu(sph):
         np.testing.assert_array_equal(bh.cpu().numpy(), [int(r[3]) for r in rows])
         np.testing.assert_array_equal(own.cpu().numpy(), [int(r[4]) for r in rows])
     ctx.close()
+
+
+# ------------------------------------------------------------------ NEXT-1, second half: per-destination lists
+@pytest.mark.parametrize("make", [lambda: wl.config(0), lambda: wl.config(1, side=33), lambda: wl.config(2, side=37),
+                                  lambda: wl.config(3, scale=0.1), lambda: wl.config(4, side=29),
+                                  lambda: wl.lattice_block(20, 20, 20, 0.1, 25, owners=("random", 32)),
+                                  lambda: wl.lattice_block(9, 9, 9, 0.1, 24, owners=("single",)),
+                                  lambda: wl.lattice_block(40, 6, 6, 0.1, 80, owners=("slabs", 3))],
+                         ids=["cfg0", "cfg1", "cfg2", "cfg3-rcb", "cfg4", "32-owners", "one-owner", "wide-slabs"])
+def test_pack_destinations_matches_oracle(sph, oracle, make):
+    """sph_pack_destinations (PAPER.md:23 step d, reading D1) against orc_pack_destinations, bit-exact:
+    offsets and every list; also the count-only call, a too-small buffer (nothing written beyond
+    its capacity, total still reported) and a second call on the same ctx (scratch re-use)."""
+    w = make()
+    g = w.n_owners
+    ctx = sph.Context.for_workload(w)
+    st = sph.State.from_numpy(w.posm, w.velr, w.sig, w.owner)
+    sh, perm = ctx.sph_sort(ctx.sph_hash(st.posm))
+    so = st.owner[perm.long()].contiguous()
+    cs, ce = ctx.sph_cell_ranges(sh)
+    torch.cuda.synchronize()
+    p = parity.u32(perm)
+    ref_off, ref_ids = oracle.pack_destinations(parity.u32(sh), w.owner[p.astype(np.int64)], p, w.dims,
+                                                parity.u32(cs), parity.u32(ce), g)
+    for rep in range(2):
+        offs, ids = ctx.sph_pack_destinations(sh, so, perm)
+        torch.cuda.synchronize()
+        np.testing.assert_array_equal(parity.u32(offs), ref_off, err_msg=f"dest_offsets (call {rep})")
+        np.testing.assert_array_equal(parity.u32(ids), ref_ids, err_msg=f"dest_ids (call {rep})")
+    # union of the lists = the boundary set stage 3 produces
+    _, bids, cnt, _ = ctx.sph_comm_hash(sh, so, perm, cs, ce)
+    torch.cuda.synchronize()
+    m = int(parity.u32(cnt)[0])
+    np.testing.assert_array_equal(np.unique(ref_ids), np.sort(parity.u32(bids)[:m]))
+    assert ref_ids.size <= m * max(g - 1, 0)
+    # a buffer that is too small: the head is written, the guard word behind it is not, the total is
+    total = int(ref_off[-1])
+    if total > 1:
+        cap = total // 2
+        buf = torch.full((cap + 1,), -1, dtype=torch.int32, device="cuda")
+        offs2, _ = ctx.sph_pack_destinations(sh, so, perm, dest_ids=buf[:cap])
+        torch.cuda.synchronize()
+        assert int(parity.u32(offs2)[-1]) == total
+        got = parity.u32(buf)
+        assert got[cap] == 0xFFFFFFFF
+        # slots below cap belong to the lists that start below cap
+        np.testing.assert_array_equal(got[:cap], ref_ids[:cap])
+    ctx.close()

@@ -98,7 +98,7 @@ def test_noalloc_refuses_grids_beyond_its_built_in_scratch():
     assert lib.sph_comm_hash_noalloc(C.byref(too_big), 0, None, None, None, C.c_void_p(8), None) == sph.SPH_ELIMIT
     huge = _params((2 ** 31 - 1, 2 ** 31 - 1, 2 ** 31 - 1))  # the product would wrap 64 bits
     assert lib.sph_comm_hash_noalloc(C.byref(huge), 0, None, None, None, C.c_void_p(8), None) == sph.SPH_ELIMIT
-    assert b"SPH_NOALLOC_MAX_CELLS" in lib.sph_strerror(sph.SPH_ELIMIT)
+    assert b"SPH_NOALLOC_MAX_CELLS" in lib.sph_strerror(sph.SPH_ELIMIT)      # the message names the limit
     ok_grid = _params((256, 128, 128))                      # exactly 2^22: passes the size check ...
     assert lib.sph_comm_hash_noalloc(C.byref(ok_grid), -1, None, None, None, C.c_void_p(8), None) == sph.SPH_EINVAL
     assert lib.sph_comm_hash_noalloc(C.byref(ok_grid), 5, None, None, None, C.c_void_p(8), None) == sph.SPH_EINVAL
