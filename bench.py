@@ -454,6 +454,10 @@ def run_ours(args, rank, world, local_rank):
         "roofline": {"kernel": "interact", "bound": "alu", "achieved": achieved_tf, "peak": fp32_peak,
                      "unit": "TFLOP/s", "frac": achieved_tf / fp32_peak,
                      "traffic": NCU_TRAFFIC_BYTES.get(args.config),
+                     "traffic_source": ("constant from the committed ncu --set full capture under profiles/ "
+                                        "(dram__bytes_read.sum + dram__bytes_write.sum per launch); not measured by this run"
+                                        if NCU_TRAFFIC_BYTES.get(args.config) else None),
+                     "algorithmic_bytes": BYTES_PER_PARTICLE["interact"] * n,
                      "peak_source": f"{props.multi_processor_count} SMs x 128 lanes x 2 x "
                                     f"{peaks['sm_max_mhz']:.0f} MHz (DESIGN.md section 7)",
                      "hbm_peak_gbs": peaks["hbm_gbs"], "hbm_peak_source": peaks["source"],

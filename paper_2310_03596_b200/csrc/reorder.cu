@@ -61,8 +61,14 @@ reorder_kernel(int64_t n, const uint32_t *__restrict__ perm, StatePtrs in, State
 // partition is stable -- and leaves as one contiguous run per label and array.  (A plain gather by
 // packed ids re-read every sector once per label, a plain scatter wrote 8-byte pieces: both
 // measured ~7 ms at 64 M boundary particles with 16 random labels.)
-constexpr int kPackTile = 1024;
-constexpr int kPackThreads = 512;
+// Tile geometry as measured at 64 M boundary particles, 16 random owners (whole sph_pack_boundary,
+// round 3): 2048 / 1024 threads 2.85 ms, 1024 / 512 2.66, 512 / 256 2.55, 384 / 192 2.53, 256 / 128
+// 2.62, 512 / 512 2.78, 256 / 256 2.48 ms (61.5 % of HBM peak).  The load and the store phase of a
+// CTA do not overlap, so many small CTAs per SM (17 KB of shared memory each) hide each other's
+// phases better than three big ones; the per-label runs of a tile (16 entries at 16 labels) are
+// still whole sectors for the 16-byte fields.
+constexpr int kPackTile = 256;
+constexpr int kPackThreads = 256;
 struct PackSmem {
     float4 posm[kPackTile], velr[kPackTile];
     float sig[6][kPackTile];
